@@ -1,0 +1,138 @@
+/*
+ * pwham.h -- C ABI of libpwham: the B200 (sm_100a) hot path of iterative Kohn-Sham diagonalisation in a
+ * plane-wave basis, after arxiv/paper_2604_11139 ("GPU acceleration of plane-wave DFT calculations in ABINIT").
+ *
+ *   H psi = 1/2|k+G|^2 psi  +  gather( FFT( V_loc(r) . iFFT( scatter(psi) ) ) )  +  P . D . (P^H psi)
+ *
+ * applied matrix-free to a block of bands ("HX(N,m)", 327-335 section 4.2, 397), inside the
+ * scaled Chebyshev polynomial filter (Algorithm 7; 246 section 3.3; 576-593 Algorithm 12 with S = I),
+ * with the Rayleigh-Ritz Gram product X^H Y as companion step (Algorithm 5 step 1; 227).
+ *
+ * Conventions
+ *   - complex128 = {re, im} pairs of IEEE doubles (== cuDoubleComplex == torch.complex128).
+ *   - A block of wavefunctions is the paper's N x M matrix, column-major: band b starts at
+ *     psi + b*ld, the plane-wave index is contiguous, ld >= npw is "the distance between two consecutive
+ *     electronic bands".  Rows >= npw of a padded column are never read or written.
+ *   - Unless a parameter says HOST, every data pointer is a DEVICE pointer owned by the caller.
+ *   - Every function returns PWH_OK (0) or a negative error code and never throws; pwh_last_error() returns a
+ *     thread-local message for the last failure.  Device work is enqueued on `stream` (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream) and is asynchronous: results are valid once the caller has
+ *     synchronised that stream.  The *_host entry points synchronise before returning.
+ *   - One handle may be used from one stream at a time.  There is no CPU fallback of any kind.
+ */
+#ifndef PWHAM_H
+#define PWHAM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pwh_ham pwh_ham; /* opaque handle */
+typedef struct {
+  double re, im;
+} pwh_c128;
+
+enum { PWH_OK = 0, PWH_EINVAL = -1, PWH_ECUDA = -2, PWH_ENOMEM = -3, PWH_EUNSUPPORTED = -4 };
+
+/*
+ * pwh_ham_setup -- build the tables of one Hamiltonian (one k-point).
+ * ("data must first be rearranged" before the batched FFT), PAPER.md:333 (projectors, D).
+ *
+ *   lattice   HOST  9 doubles, row i = primitive vector a_i in bohr.
+ *   kpt       HOST  3 doubles, reduced coordinates of k.
+ *   fft_dims  HOST  n1, n2, n3; each must be >= 2 with prime factors in {2,3,5} (else PWH_EUNSUPPORTED).
+ *   npw       number of plane waves N (>= 1).
+ *   gvec      DEVICE int32 [npw][3], reduced integer components of G.  The set must fit the box without
+ *             collision after wrapping (n mod n_i); checked once here (one device->host copy). Copied.
+ *   vloc      DEVICE double [n1*n2*n3], local potential in Hartree on the real-space grid, index
+ *             i1 + n1*(i2 + n2*i3).  Copied (re-ordered and pre-scaled by 1/(n1 n2 n3)) into the handle.
+ *   nproj     number of projectors J (>= 0; 0 disables the nonlocal term).
+ *   proj      DEVICE complex128, column-major npw x nproj, proj[g + i*ldp] = <G_g | p_i>.  BORROWED: it must stay
+ *             valid and unchanged for the handle's lifetime (it can be several GB and is not copied).
+ *   ldp       leading dimension of proj (>= npw).
+ *   dij       DEVICE double [nproj], diagonal nonlocal strengths D_i in Hartree.  Copied.
+ *   stream    stream used for the setup copies; the call synchronises it before returning.
+ *
+ * The kinetic diagonal is kin(G) = 1/2 |B(k + n_G)|^2 with B = 2 pi (A^-1)^T.
+ */
+int pwh_ham_setup(pwh_ham** out, const double lattice[9], const double kpt[3], const int32_t fft_dims[3],
+                  int64_t npw, const int32_t* gvec, const double* vloc, int64_t nproj, const pwh_c128* proj,
+                  int64_t ldp, const double* dij, void* stream);
+
+/* Frees the handle's tables and any staging buffers of the *_host entry points.  NULL is accepted. */
+int pwh_ham_destroy(pwh_ham* ham);
+
+/* Bytes of caller-provided device workspace that pwh_apply_h / pwh_cheb_filter need for up to nband_max bands.
+ * The hot path performs no allocation. */
+size_t pwh_workspace_bytes(const pwh_ham* ham, int64_t nband_max);
+
+/*
+ * pwh_apply_h -- hpsi = H psi for nband bands (HX(N,m); the three terms PAPER.md:397).
+ *   psi [in]  npw x nband, leading dimension ldpsi.   hpsi [out] npw x nband, leading dimension ldh.
+ *   psi and hpsi must not overlap.  ws/ws_bytes: workspace of at least pwh_workspace_bytes(ham, nband), 256-byte
+ *   aligned.  nband == 0 is a no-op.
+ * Errors: PWH_EINVAL (null pointer, ld < npw, workspace too small or misaligned), PWH_ECUDA (launch failure).
+ */
+int pwh_apply_h(pwh_ham* ham, int64_t nband, const pwh_c128* psi, int64_t ldpsi, pwh_c128* hpsi, int64_t ldh,
+                void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * pwh_cheb_filter -- in place psi <- p_m(H) psi, the scaled Chebyshev filter of degree m = `degree`
+ * (Algorithm 7 loop body, 246; recurrence of the paper's reference [61]):
+ *     e = (b-a)/2,  c = (b+a)/2,  sigma_1 = e/(a0-c),  Y_0 = psi,  Y_1 = (sigma_1/e)(H - c) Y_0,
+ *     sigma_{j+1} = 1/(2/sigma_1 - sigma_j),   Y_{j+1} = (2 sigma_{j+1}/e)(H - c) Y_j - sigma_j sigma_{j+1} Y_{j-1},
+ * result Y_m = T_m((H-c)/e)/T_m((a0-c)/e) psi.  [a,b] is the damped interval, a0 < a the normalisation point.
+ * One H application per degree.  degree == 0 is the identity.
+ * Errors: PWH_EINVAL additionally for degree < 0, b <= a, a0 >= a.
+ */
+int pwh_cheb_filter(pwh_ham* ham, int64_t nband, pwh_c128* psi, int64_t ld, int degree, double a, double b,
+                    double a0, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * pwh_gram -- G = X^H Y  (Algorithm 5 step 1 with Y = H X; PAPER.md:227 writes it as a sum of
+ * row-chunk products, which is how it is evaluated here: split over npw with a fixed-order second-stage sum, so
+ * the result is deterministic).
+ *   X npw x nx (ldx), Y npw x ny (ldy), G [out] column-major nx x ny (ldg >= nx): G[i + j*ldg] = sum_g conj(X[g,i]) Y[g,j].
+ *   ws/ws_bytes: at least pwh_gram_workspace_bytes(npw, nx, ny), 256-byte aligned.
+ */
+size_t pwh_gram_workspace_bytes(int64_t npw, int64_t nx, int64_t ny);
+int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny, const pwh_c128* Y, int64_t ldy,
+             pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * Host-buffer entry points (end-to-end path: the paper keeps Psi on the device and moves it host->device once per
+ * k-point and SCF step, Algorithm 3).  All pointers below marked HOST are host memory (pinned
+ * memory gives asynchronous copies; pageable memory works).  Device staging buffers are allocated on first use,
+ * cached in the handle and freed by pwh_ham_destroy.  Each call copies its inputs to the device, runs the same
+ * kernels as the device entry points, copies the result back and synchronises.
+ *
+ * pwh_apply_h_host     hpsi_host = H psi_host.
+ * pwh_cheb_filter_host psi_host <- p_m(H) psi_host, bands processed in column blocks of `block` (<= 0: all at once).
+ * pwh_sweep_host       one filtering sweep followed by the Rayleigh-Ritz projection: psi_host <- p_m(H) psi_host
+ *                      (by blocks), then G_host = psi^H (H psi) (column-major nband x nband, ldg) -- i.e. degree+1
+ *                      H applications per band and one Gram product.  hpsi_host (optional, may be NULL) receives H psi.
+ */
+int pwh_apply_h_host(pwh_ham* ham, int64_t nband, const pwh_c128* psi_host, int64_t ldpsi, pwh_c128* hpsi_host,
+                     int64_t ldh, void* stream);
+int pwh_cheb_filter_host(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
+                         double a, double b, double a0, void* stream);
+int pwh_sweep_host(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree, double a,
+                   double b, double a0, pwh_c128* hpsi_host, int64_t ldh, pwh_c128* G_host, int64_t ldg,
+                   void* stream);
+
+/* Number of kernel launches issued by this library since load (all handles, all threads). */
+int64_t pwh_launch_count(void);
+
+/* Introspection: fills info[0..7] = {npw, nproj, n1, n2, n3, n_zcolumns, n_xlines, reserved}. */
+int pwh_ham_info(const pwh_ham* ham, int64_t info[8]);
+
+/* Thread-local message describing the last error returned on this thread ("" if none). */
+const char* pwh_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PWHAM_H */

@@ -1,0 +1,284 @@
+"""Thin ctypes binding over libpwham.so (C ABI in include/pwham.h) -- argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch is used here for device memory and streams
+and nothing else.  There is no CPU fallback: importing works without a GPU (so that the symbol table can be
+checked), but every compute entry point needs CUDA tensors, and loading fails loudly if the library has not
+been built (`python paper_2604_11139_b200/build.py` or `__graft_entry__.build()`).
+
+Array conventions (see synth.py): a block is a complex128 tensor of shape (nband, npw) whose rows are bands, i.e. the
+paper's N x M matrix Psi column-major with leading dimension `stride(0)`.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpwham.so")
+
+EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply_h", "pwh_cheb_filter",
+           "pwh_gram_workspace_bytes", "pwh_gram", "pwh_apply_h_host", "pwh_cheb_filter_host", "pwh_sweep_host",
+           "pwh_launch_count", "pwh_ham_info", "pwh_last_error"]
+
+_lib = None
+
+
+class PwhamError(RuntimeError):
+    pass
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libpwham.so and declare the prototypes of include/pwham.h.  Raises if the library is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise PwhamError(f"{LIB_PATH} is missing: build the CUDA library first (python paper_2604_11139_b200/build.py "
+                         "or __graft_entry__.build()); there is no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i64, i32, dbl, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    L.pwh_ham_setup.argtypes = [ctypes.POINTER(vp), vp, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp]
+    L.pwh_ham_setup.restype = i32
+    L.pwh_ham_destroy.argtypes = [vp]
+    L.pwh_ham_destroy.restype = i32
+    L.pwh_workspace_bytes.argtypes = [vp, i64]
+    L.pwh_workspace_bytes.restype = sz
+    L.pwh_apply_h.argtypes = [vp, i64, vp, i64, vp, i64, vp, sz, vp]
+    L.pwh_apply_h.restype = i32
+    L.pwh_cheb_filter.argtypes = [vp, i64, vp, i64, i32, dbl, dbl, dbl, vp, sz, vp]
+    L.pwh_cheb_filter.restype = i32
+    L.pwh_gram_workspace_bytes.argtypes = [i64, i64, i64]
+    L.pwh_gram_workspace_bytes.restype = sz
+    L.pwh_gram.argtypes = [i64, i64, vp, i64, i64, vp, i64, vp, i64, vp, sz, vp]
+    L.pwh_gram.restype = i32
+    L.pwh_apply_h_host.argtypes = [vp, i64, vp, i64, vp, i64, vp]
+    L.pwh_apply_h_host.restype = i32
+    L.pwh_cheb_filter_host.argtypes = [vp, i64, i64, vp, i64, i32, dbl, dbl, dbl, vp]
+    L.pwh_cheb_filter_host.restype = i32
+    L.pwh_sweep_host.argtypes = [vp, i64, i64, vp, i64, i32, dbl, dbl, dbl, vp, i64, vp, i64, vp]
+    L.pwh_sweep_host.restype = i32
+    L.pwh_launch_count.argtypes = []
+    L.pwh_launch_count.restype = i64
+    L.pwh_ham_info.argtypes = [vp, vp]
+    L.pwh_ham_info.restype = i32
+    L.pwh_last_error.argtypes = []
+    L.pwh_last_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        msg = load_library().pwh_last_error().decode("utf-8", "replace")
+        raise PwhamError(f"{what} failed with code {rc}: {msg}")
+
+
+def _stream_ptr(device) -> int:
+    return int(torch.cuda.current_stream(device).cuda_stream)
+
+
+def _dev_tensor(x, dtype, device) -> torch.Tensor:
+    if isinstance(x, np.ndarray):
+        x = torch.from_numpy(np.ascontiguousarray(x))
+    return x.to(device=device, dtype=dtype).contiguous()
+
+
+def _block_args(t: torch.Tensor, npw: int, name: str):
+    if not (t.is_cuda and t.dtype == torch.complex128 and t.dim() == 2):
+        raise PwhamError(f"{name} must be a 2-D CUDA complex128 tensor of shape (nband, npw)")
+    if t.shape[1] != npw or t.stride(1) != 1 or (t.shape[0] > 1 and t.stride(0) < npw):
+        raise PwhamError(f"{name}: expected shape (nband, {npw}) with unit stride along plane waves")
+    ld = t.stride(0) if t.shape[0] > 1 else max(npw, t.stride(0))
+    return t.data_ptr(), int(ld)
+
+
+class Ham:
+    """Owner of one pwh_ham handle plus the device tensors it borrows (projectors) and its cached workspace."""
+
+    def __init__(self, handle: int, device, npw: int, nproj: int, keep):
+        self.handle = ctypes.c_void_p(handle)
+        self.device = device
+        self.npw = npw
+        self.nproj = nproj
+        self._keep = keep
+        self._ws: Optional[torch.Tensor] = None
+
+    def workspace(self, nband: int) -> torch.Tensor:
+        need = int(load_library().pwh_workspace_bytes(self.handle, nband))
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=self.device)
+        return self._ws
+
+    def info(self) -> dict:
+        arr = (ctypes.c_int64 * 8)()
+        _check(load_library().pwh_ham_info(self.handle, arr), "pwh_ham_info")
+        keys = ["npw", "nproj", "n1", "n2", "n3", "n_zcolumns", "n_xlines", "band_group"]
+        return dict(zip(keys, [int(v) for v in arr]))
+
+    def destroy(self) -> None:
+        if self.handle:
+            load_library().pwh_ham_destroy(self.handle)
+            self.handle = ctypes.c_void_p(None)
+            self._keep = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def ham_setup(lattice, kpt, fft_dims, gvec, vloc, proj, dij, device="cuda:0") -> Ham:
+    """pwh_ham_setup: build the handle.  gvec (npw,3) int32, vloc (n3,n2,n1) float64, proj (nproj,npw) complex128
+    (row i = <G|p_i>, i.e. column-major npw x nproj), dij (nproj,) float64; numpy arrays or torch tensors."""
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise PwhamError("CUDA is not available: libpwham has no CPU fallback")
+    device = torch.device(device)
+    lattice = np.ascontiguousarray(np.asarray(lattice, dtype=np.float64).reshape(9))
+    kpt = np.ascontiguousarray(np.asarray(kpt, dtype=np.float64).reshape(3))
+    dims = np.ascontiguousarray(np.asarray(fft_dims, dtype=np.int32).reshape(3))
+    g = _dev_tensor(gvec, torch.int32, device)
+    npw = int(g.shape[0])
+    v = _dev_tensor(vloc, torch.float64, device)
+    if tuple(v.shape) != (int(dims[2]), int(dims[1]), int(dims[0])):
+        raise PwhamError("vloc must have shape (n3, n2, n1)")
+    if proj is None or len(proj) == 0:
+        nproj, p, d, p_ptr, d_ptr, ldp = 0, None, None, None, None, npw
+    else:
+        p = _dev_tensor(proj, torch.complex128, device)
+        d = _dev_tensor(dij, torch.float64, device)
+        nproj = int(p.shape[0])
+        if p.shape[1] != npw or d.shape[0] != nproj:
+            raise PwhamError("proj must be (nproj, npw) and dij (nproj,)")
+        p_ptr, d_ptr, ldp = p.data_ptr(), d.data_ptr(), npw
+    handle = ctypes.c_void_p()
+    with torch.cuda.device(device):
+        rc = L.pwh_ham_setup(ctypes.byref(handle), lattice.ctypes.data, kpt.ctypes.data, dims.ctypes.data, npw,
+                             g.data_ptr(), v.data_ptr(), nproj, p_ptr, ldp, d_ptr, _stream_ptr(device))
+    _check(rc, "pwh_ham_setup")
+    return Ham(handle.value, device, npw, nproj, keep=(p,))
+
+
+def ham_destroy(ham: Ham) -> None:
+    ham.destroy()
+
+
+def apply_h(ham: Ham, psi: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """pwh_apply_h: out = H psi for a block psi (nband, npw)."""
+    L = load_library()
+    p_ptr, ldp = _block_args(psi, ham.npw, "psi")
+    if out is None:
+        out = torch.empty((psi.shape[0], ham.npw), dtype=torch.complex128, device=psi.device)
+    o_ptr, ldo = _block_args(out, ham.npw, "out")
+    nband = int(psi.shape[0])
+    ws = ham.workspace(nband)
+    with torch.cuda.device(ham.device):
+        rc = L.pwh_apply_h(ham.handle, nband, p_ptr, ldp, o_ptr, ldo, ws.data_ptr(), ws.numel(), _stream_ptr(ham.device))
+    _check(rc, "pwh_apply_h")
+    return out
+
+
+def cheb_filter(ham: Ham, psi: torch.Tensor, degree: int, a: float, b: float, a0: float) -> torch.Tensor:
+    """pwh_cheb_filter: in place psi <- T_m((H-c)/e)/T_m((a0-c)/e) psi; returns psi."""
+    L = load_library()
+    p_ptr, ld = _block_args(psi, ham.npw, "psi")
+    nband = int(psi.shape[0])
+    ws = ham.workspace(nband)
+    with torch.cuda.device(ham.device):
+        rc = L.pwh_cheb_filter(ham.handle, nband, p_ptr, ld, int(degree), float(a), float(b), float(a0), ws.data_ptr(),
+                               ws.numel(), _stream_ptr(ham.device))
+    _check(rc, "pwh_cheb_filter")
+    return psi
+
+
+_gram_ws = {}
+
+
+def gram(x: torch.Tensor, y: torch.Tensor) -> torch.Tensor:
+    """pwh_gram: returns G of shape (nx, ny) with G[i, j] = <x_i, y_j> = sum_g conj(x[i, g]) y[j, g]."""
+    L = load_library()
+    npw = int(x.shape[1])
+    x_ptr, ldx = _block_args(x, npw, "x")
+    y_ptr, ldy = _block_args(y, npw, "y")
+    nx, ny = int(x.shape[0]), int(y.shape[0])
+    g_cm = torch.empty((ny, nx), dtype=torch.complex128, device=x.device)   # column-major nx x ny
+    need = int(L.pwh_gram_workspace_bytes(npw, nx, ny))
+    key = (x.device.index, )
+    ws = _gram_ws.get(key)
+    if ws is None or ws.numel() < need:
+        _gram_ws[key] = None
+        ws = _gram_ws[key] = torch.empty(need, dtype=torch.uint8, device=x.device)
+    with torch.cuda.device(x.device):
+        rc = L.pwh_gram(npw, nx, x_ptr, ldx, ny, y_ptr, ldy, g_cm.data_ptr(), nx, ws.data_ptr(), ws.numel(),
+                        _stream_ptr(x.device))
+    _check(rc, "pwh_gram")
+    return g_cm.T
+
+
+def _host_block(a, npw: int, name: str):
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.complex128 or a.dim() != 2 or a.shape[1] != npw or not a.is_contiguous():
+            raise PwhamError(f"{name} must be a contiguous host complex128 tensor (nband, npw)")
+        return a.data_ptr(), int(a.shape[0])
+    if not (isinstance(a, np.ndarray) and a.dtype == np.complex128 and a.ndim == 2 and a.shape[1] == npw
+            and a.flags.c_contiguous):
+        raise PwhamError(f"{name} must be a C-contiguous host complex128 array (nband, npw)")
+    return a.ctypes.data, int(a.shape[0])
+
+
+def apply_h_host(ham: Ham, psi_host, hpsi_host) -> None:
+    """pwh_apply_h_host: host buffers in, host buffers out (copies inside the call)."""
+    L = load_library()
+    p, nband = _host_block(psi_host, ham.npw, "psi_host")
+    o, nb2 = _host_block(hpsi_host, ham.npw, "hpsi_host")
+    if nb2 != nband:
+        raise PwhamError("psi_host / hpsi_host band counts differ")
+    with torch.cuda.device(ham.device):
+        rc = L.pwh_apply_h_host(ham.handle, nband, p, ham.npw, o, ham.npw, _stream_ptr(ham.device))
+    _check(rc, "pwh_apply_h_host")
+
+
+def cheb_filter_host(ham: Ham, psi_host, degree: int, a: float, b: float, a0: float, block: int = 0) -> None:
+    """pwh_cheb_filter_host: in place on a host block, bands filtered in column blocks of `block`."""
+    L = load_library()
+    p, nband = _host_block(psi_host, ham.npw, "psi_host")
+    with torch.cuda.device(ham.device):
+        rc = L.pwh_cheb_filter_host(ham.handle, nband, int(block), p, ham.npw, int(degree), float(a), float(b),
+                                    float(a0), _stream_ptr(ham.device))
+    _check(rc, "pwh_cheb_filter_host")
+
+
+def sweep_host(ham: Ham, psi_host, degree: int, a: float, b: float, a0: float, g_host, block: int = 0,
+               hpsi_host=None) -> None:
+    """pwh_sweep_host: psi_host <- p_m(H) psi_host, then g_host (nband, nband; g_host[j, i] = <psi_i, H psi_j>,
+    i.e. the column-major Gram matrix) -- degree+1 H applications per band and one Gram product, host to host."""
+    L = load_library()
+    p, nband = _host_block(psi_host, ham.npw, "psi_host")
+    if isinstance(g_host, torch.Tensor):
+        g_ptr, ok = g_host.data_ptr(), (g_host.dtype == torch.complex128 and tuple(g_host.shape) == (nband, nband)
+                                        and g_host.is_contiguous() and not g_host.is_cuda)
+    else:
+        g_ptr, ok = g_host.ctypes.data, (g_host.dtype == np.complex128 and g_host.shape == (nband, nband)
+                                         and g_host.flags.c_contiguous)
+    if not ok:
+        raise PwhamError("g_host must be a contiguous host complex128 (nband, nband) array")
+    h_ptr = None
+    if hpsi_host is not None:
+        h_ptr, nb2 = _host_block(hpsi_host, ham.npw, "hpsi_host")
+        if nb2 != nband:
+            raise PwhamError("hpsi_host band count differs")
+    with torch.cuda.device(ham.device):
+        rc = L.pwh_sweep_host(ham.handle, nband, int(block), p, ham.npw, int(degree), float(a), float(b), float(a0),
+                              h_ptr, ham.npw, g_ptr, nband, _stream_ptr(ham.device))
+    _check(rc, "pwh_sweep_host")
+
+
+def launch_count() -> int:
+    return int(load_library().pwh_launch_count())

@@ -1,0 +1,621 @@
+// pwham.cu -- C ABI of libpwham (include/pwham.h): handle setup, workspace carving and the launch sequences of
+// apply_h, cheb_filter and gram.  Host code here only builds tables and enqueues kernels; every step of the path
+// (scatter, FFTs, V_loc multiply, gather, kinetic, recurrence, projector and Gram contractions) runs in the
+// kernels of local_kernels.cu and zgemm.cu.  There is no CPU fallback.
+#include "../../include/pwham.h"
+
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "launch.h"
+
+using namespace pwh;
+
+namespace pwh {
+static std::atomic<int64_t> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+}  // namespace pwh
+
+static thread_local std::string g_err;
+
+static int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                        \
+  do {                                                                                        \
+    cudaError_t e__ = (expr);                                                                 \
+    if (e__ != cudaSuccess)                                                                   \
+      return fail(e__ == cudaErrorMemoryAllocation ? PWH_ENOMEM : PWH_ECUDA, "%s: %s", #expr, \
+                  cudaGetErrorString(e__));                                                   \
+  } while (0)
+
+struct pwh_ham {
+  int64_t npw = 0, nproj = 0;
+  int n1 = 0, n2 = 0, n3 = 0;
+  LocalPlan lp;
+  const c128* proj = nullptr;
+  int64_t ldp = 0;
+  double* dij = nullptr;
+  int band_group = 1;
+  std::vector<void*> allocs;
+  // staging of the *_host entry points
+  void* st_psi = nullptr;
+  void* st_hpsi = nullptr;
+  void* st_g = nullptr;
+  void* st_ws = nullptr;
+  size_t st_psi_bytes = 0, st_hpsi_bytes = 0, st_g_bytes = 0, st_ws_bytes = 0;
+};
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ---------------------------------------------------------------------------------------------------------------
+// setup helpers
+// ---------------------------------------------------------------------------------------------------------------
+static bool factor_235(int n, int& e2, int& e3, int& e5) {
+  e2 = e3 = e5 = 0;
+  while (n % 2 == 0) { n /= 2; ++e2; }
+  while (n % 3 == 0) { n /= 3; ++e3; }
+  while (n % 5 == 0) { n /= 5; ++e5; }
+  return n == 1;
+}
+
+// radix schedule: 8s, 4s, 5s, 3s, then a lone 2 (8*2 is re-split into 4*4)
+static bool make_axis_plan(int n, AxisPlan& pl, std::vector<c128>& tw, std::vector<int>& nat) {
+  int e2, e3, e5;
+  if (n < 2 || !factor_235(n, e2, e3, e5)) return false;
+  std::vector<int> rad;
+  int n8 = e2 / 3, rem = e2 % 3, n4 = 0, n2 = 0;
+  if (rem == 1) {
+    if (n8 >= 1) { --n8; n4 += 2; } else n2 = 1;
+  } else if (rem == 2) n4 += 1;
+  for (int i = 0; i < n8; ++i) rad.push_back(8);
+  for (int i = 0; i < n4; ++i) rad.push_back(4);
+  for (int i = 0; i < e5; ++i) rad.push_back(5);
+  for (int i = 0; i < e3; ++i) rad.push_back(3);
+  for (int i = 0; i < n2; ++i) rad.push_back(2);
+  if ((int)rad.size() > PWH_MAX_STAGES) return false;
+  memset(&pl, 0, sizeof(pl));
+  pl.n = n;
+  pl.nstages = (int)rad.size();
+  tw.clear();
+  int B = n;
+  const long double PI = 3.14159265358979323846264338327950288L;
+  for (int s = 0; s < pl.nstages; ++s) {
+    const int r = rad[s], m = B / r;
+    pl.radix[s] = r;
+    pl.m[s] = m;
+    pl.div_m[s] = make_fastdiv((uint32_t)m);
+    pl.tw_off[s] = (int)tw.size();
+    if (m > 1) {
+      for (int k = 1; k < r; ++k)
+        for (int n2i = 0; n2i < m; ++n2i) {
+          const long t = ((long)n2i * k) % B;
+          const long double ang = 2.0L * PI * (long double)t / (long double)B;
+          tw.push_back(cmake((double)cosl(ang), (double)sinl(ang)));
+        }
+    }
+    B = m;
+  }
+  pl.tw_len = (int)tw.size();
+  // position -> natural index of the digit-permuted order
+  nat.assign(n, 0);
+  std::vector<int> cur(1, 0);
+  int size = 1;
+  for (int s = pl.nstages - 1; s >= 0; --s) {
+    const int r = rad[s];
+    std::vector<int> next((size_t)size * r);
+    for (int k1 = 0; k1 < r; ++k1)
+      for (int p = 0; p < size; ++p) next[(size_t)k1 * size + p] = k1 + r * cur[p];
+    cur.swap(next);
+    size *= r;
+  }
+  nat = cur;
+  return true;
+}
+
+__global__ void k_permute_vloc(int n1, int n2, int n3, const double* __restrict__ v, const int* __restrict__ natx,
+                               const int* __restrict__ naty, const int* __restrict__ natz, double inv_f,
+                               double* __restrict__ out) {
+  const int64_t total = (int64_t)n1 * n2 * n3;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int px = (int)(i % n1);
+    const int py = (int)((i / n1) % n2);
+    const int pz = (int)(i / ((int64_t)n1 * n2));
+    out[i] = v[natx[px] + (int64_t)n1 * (naty[py] + (int64_t)n2 * natz[pz])] * inv_f;
+  }
+}
+
+template <typename T>
+static int upload(pwh_ham* h, const std::vector<T>& v, const T** out, cudaStream_t st) {
+  void* d = nullptr;
+  const size_t bytes = std::max<size_t>(v.size() * sizeof(T), 16);
+  CUDA_TRY(cudaMalloc(&d, bytes));
+  h->allocs.push_back(d);
+  if (!v.empty()) CUDA_TRY(cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+  *out = reinterpret_cast<const T*>(d);
+  return PWH_OK;
+}
+
+static int wrapi(int v, int n) {
+  int r = v % n;
+  return r < 0 ? r + n : r;
+}
+
+extern "C" int pwh_ham_destroy(pwh_ham* h) {
+  if (!h) return PWH_OK;
+  for (void* p : h->allocs) cudaFree(p);
+  if (h->st_psi) cudaFree(h->st_psi);
+  if (h->st_hpsi) cudaFree(h->st_hpsi);
+  if (h->st_g) cudaFree(h->st_g);
+  if (h->st_ws) cudaFree(h->st_ws);
+  delete h;
+  return PWH_OK;
+}
+
+static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], const int32_t dims[3], int64_t npw,
+                      const int32_t* gvec, const double* vloc, int64_t nproj, const pwh_c128* proj, int64_t ldp,
+                      const double* dij, cudaStream_t st) {
+  const int n1 = dims[0], n2 = dims[1], n3 = dims[2];
+  h->npw = npw;
+  h->nproj = nproj;
+  h->n1 = n1; h->n2 = n2; h->n3 = n3;
+  h->proj = reinterpret_cast<const c128*>(proj);
+  h->ldp = ldp;
+  LocalPlan& lp = h->lp;
+  memset(&lp, 0, sizeof(lp));
+  lp.n1 = n1; lp.n2 = n2; lp.n3 = n3;
+
+  // FFT plans
+  std::vector<c128> tw[3];
+  std::vector<int> nat[3];
+  for (int ax = 0; ax < 3; ++ax)
+    if (!make_axis_plan(dims[ax], lp.ax[ax], tw[ax], nat[ax]))
+      return fail(PWH_EUNSUPPORTED, "fft_dims[%d] = %d: only sizes >= 2 with prime factors 2, 3, 5 are supported", ax,
+                  dims[ax]);
+  if (n1 > 4096 || n2 > 4096 || n3 > 4096) return fail(PWH_EUNSUPPORTED, "fft_dims larger than 4096 not supported");
+
+  // G vectors to the host (once), validation
+  std::vector<int32_t> g((size_t)npw * 3);
+  CUDA_TRY(cudaMemcpyAsync(g.data(), gvec, g.size() * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  const size_t F = (size_t)n1 * n2 * n3;
+  {
+    std::vector<bool> seen(F, false);
+    for (int64_t i = 0; i < npw; ++i) {
+      const size_t idx = wrapi(g[3 * i], n1) + (size_t)n1 * (wrapi(g[3 * i + 1], n2) + (size_t)n2 * wrapi(g[3 * i + 2], n3));
+      if (seen[idx]) return fail(PWH_EINVAL, "gvec: plane wave %lld collides with another one in the FFT box", (long long)i);
+      seen[idx] = true;
+    }
+  }
+
+  // kinetic diagonal 1/2 |B (k + n)|^2, B = 2 pi (A^-1)^T
+  {
+    const double* a = lattice;
+    const double det = a[0] * (a[4] * a[8] - a[5] * a[7]) - a[1] * (a[3] * a[8] - a[5] * a[6]) +
+                       a[2] * (a[3] * a[7] - a[4] * a[6]);
+    if (!(std::fabs(det) > 0.0)) return fail(PWH_EINVAL, "lattice is singular");
+    const double tp = 6.283185307179586476925286766559 / det;
+    const double b1[3] = {tp * (a[4] * a[8] - a[5] * a[7]), tp * (a[5] * a[6] - a[3] * a[8]), tp * (a[3] * a[7] - a[4] * a[6])};
+    const double b2[3] = {tp * (a[7] * a[2] - a[8] * a[1]), tp * (a[8] * a[0] - a[6] * a[2]), tp * (a[6] * a[1] - a[7] * a[0])};
+    const double b3[3] = {tp * (a[1] * a[5] - a[2] * a[4]), tp * (a[2] * a[3] - a[0] * a[5]), tp * (a[0] * a[4] - a[1] * a[3])};
+    std::vector<double> kin((size_t)npw);
+    for (int64_t i = 0; i < npw; ++i) {
+      const double c0 = kpt[0] + g[3 * i], c1 = kpt[1] + g[3 * i + 1], c2 = kpt[2] + g[3 * i + 2];
+      double q2 = 0.0;
+      for (int d = 0; d < 3; ++d) {
+        const double q = c0 * b1[d] + c1 * b2[d] + c2 * b3[d];
+        q2 += q * q;
+      }
+      kin[i] = 0.5 * q2;
+    }
+    int rc = upload(h, kin, &lp.kin, st);
+    if (rc) return rc;
+  }
+
+  // z-columns touched by the sphere, ordered by the signed (gy, gx) of their first member
+  struct Col { int xw, yw, gx, gy; };
+  std::vector<int> col_of_xy((size_t)n1 * n2, -1);
+  std::vector<Col> cols;
+  for (int64_t i = 0; i < npw; ++i) {
+    const int xw = wrapi(g[3 * i], n1), yw = wrapi(g[3 * i + 1], n2);
+    int& c = col_of_xy[(size_t)yw * n1 + xw];
+    if (c < 0) {
+      c = (int)cols.size();
+      cols.push_back({xw, yw, g[3 * i], g[3 * i + 1]});
+    }
+  }
+  std::vector<int> order(cols.size());
+  for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+  std::sort(order.begin(), order.end(), [&](int a_, int b_) {
+    const Col &A = cols[a_], &B = cols[b_];
+    return A.gy != B.gy ? A.gy < B.gy : (A.gx != B.gx ? A.gx < B.gx : a_ < b_);
+  });
+  std::vector<int> rank(cols.size());
+  for (size_t r = 0; r < order.size(); ++r) rank[order[r]] = (int)r;
+  const int ncols = (int)cols.size();
+
+  // x-lines touched, ordered by signed gx
+  std::vector<int> xl_gx(n1, INT32_MAX);
+  for (const Col& c : cols) xl_gx[c.xw] = std::min(xl_gx[c.xw], c.gx);
+  std::vector<int> xs;
+  for (int x = 0; x < n1; ++x)
+    if (xl_gx[x] != INT32_MAX) xs.push_back(x);
+  std::sort(xs.begin(), xs.end(), [&](int a_, int b_) { return xl_gx[a_] != xl_gx[b_] ? xl_gx[a_] < xl_gx[b_] : a_ < b_; });
+  const int nxl = (int)xs.size();
+  std::vector<short> xl_of_x(n1, -1), x_of_xl(nxl);
+  for (int i = 0; i < nxl; ++i) { xl_of_x[xs[i]] = (short)i; x_of_xl[i] = (short)xs[i]; }
+
+  lp.ncols = ncols;
+  lp.nxl = nxl;
+  lp.colgrp = 16;
+  lp.ngrp = (ncols + lp.colgrp - 1) / lp.colgrp;
+  lp.ncols_pad = lp.ngrp * lp.colgrp;
+  lp.zstride = n3 | 1;
+  lp.ystride = n2 | 1;
+  lp.xstride = n1 | 1;
+  int xb = 1;
+  for (int d = 1; d <= 32 && d <= n2; ++d)
+    if (n2 % d == 0) xb = d;
+  lp.xbatch = xb;
+  lp.div_colgrp = make_fastdiv(lp.colgrp);
+  lp.div_nxl = make_fastdiv(nxl);
+  lp.div_xbatch = make_fastdiv(xb);
+  lp.div_n1 = make_fastdiv(n1);
+  lp.div_ncols_pad = make_fastdiv(lp.ncols_pad);
+
+  std::vector<int> col_hp(lp.ncols_pad, -1);
+  for (size_t i = 0; i < cols.size(); ++i) col_hp[rank[i]] = xl_of_x[cols[i].xw] * lp.ystride + cols[i].yw;
+
+  // sphere entries sorted by (column group, plane-wave index)
+  std::vector<int> ent_grp((size_t)npw), ent_off((size_t)npw), perm((size_t)npw);
+  for (int64_t i = 0; i < npw; ++i) {
+    const int xw = wrapi(g[3 * i], n1), yw = wrapi(g[3 * i + 1], n2), zw = wrapi(g[3 * i + 2], n3);
+    const int c = rank[col_of_xy[(size_t)yw * n1 + xw]];
+    ent_grp[i] = c / lp.colgrp;
+    ent_off[i] = (c % lp.colgrp) * lp.zstride + zw;
+    perm[i] = (int)i;
+  }
+  std::stable_sort(perm.begin(), perm.end(), [&](int a_, int b_) { return ent_grp[a_] < ent_grp[b_]; });
+  std::vector<int> grp_ptr(lp.ngrp + 1, 0), ent_pw_s((size_t)npw), ent_off_s((size_t)npw);
+  for (int64_t e = 0; e < npw; ++e) {
+    ent_pw_s[e] = perm[e];
+    ent_off_s[e] = ent_off[perm[e]];
+    grp_ptr[ent_grp[perm[e]] + 1]++;
+  }
+  for (int gi = 0; gi < lp.ngrp; ++gi) grp_ptr[gi + 1] += grp_ptr[gi];
+
+  int rc;
+  if ((rc = upload(h, grp_ptr, &lp.grp_ptr, st))) return rc;
+  if ((rc = upload(h, ent_pw_s, &lp.ent_pw, st))) return rc;
+  if ((rc = upload(h, ent_off_s, &lp.ent_off, st))) return rc;
+  if ((rc = upload(h, col_hp, &lp.col_hp, st))) return rc;
+  if ((rc = upload(h, xl_of_x, &lp.xl_of_x, st))) return rc;
+  if ((rc = upload(h, x_of_xl, &lp.x_of_xl, st))) return rc;
+  for (int ax = 0; ax < 3; ++ax)
+    if ((rc = upload(h, tw[ax], &lp.tw[ax], st))) return rc;
+  {
+    std::vector<AxisPlan> plans(lp.ax, lp.ax + 3);
+    if ((rc = upload(h, plans, &lp.axp, st))) return rc;
+  }
+
+  // V_loc / F in digit-permuted positions
+  {
+    const int* dnat[3];
+    for (int ax = 0; ax < 3; ++ax)
+      if ((rc = upload(h, nat[ax], &dnat[ax], st))) return rc;
+    double* vp = nullptr;
+    CUDA_TRY(cudaMalloc(&vp, F * sizeof(double)));
+    h->allocs.push_back(vp);
+    k_permute_vloc<<<148 * 4, 256, 0, st>>>(n1, n2, n3, vloc, dnat[0], dnat[1], dnat[2], 1.0 / (double)F, vp);
+    CUDA_TRY(cudaGetLastError());
+    lp.vperm = vp;
+  }
+
+  // D (copied)
+  if (nproj > 0) {
+    CUDA_TRY(cudaMalloc(&h->dij, nproj * sizeof(double)));
+    h->allocs.push_back(h->dij);
+    CUDA_TRY(cudaMemcpyAsync(h->dij, dij, nproj * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  }
+
+  // shared-memory budgets
+  int dev = 0, smem_max = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  if (plane_smem(lp) > (size_t)smem_max || zkernel_smem(lp) > (size_t)smem_max)
+    return fail(PWH_EUNSUPPORTED, "FFT box %dx%dx%d needs %zu bytes of shared memory per plane (limit %d)", n1, n2, n3,
+                plane_smem(lp), smem_max);
+  CUDA_TRY(local_kernels_init(lp));
+  CUDA_TRY(zgemm_init());
+
+  // bands per launch of the local kernels: keep the column buffer around 48 MB (L2-resident) but at least 2 waves
+  const size_t per_band = (size_t)n3 * lp.ncols_pad * sizeof(c128);
+  int64_t grp = (int64_t)((48u << 20) / std::max<size_t>(per_band, 1));
+  const int64_t min_grp = (2 * 148 + n3 - 1) / n3;
+  grp = std::max<int64_t>(grp, min_grp);
+  grp = std::min<int64_t>(std::max<int64_t>(grp, 1), 4096);
+  h->band_group = (int)grp;
+
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return PWH_OK;
+}
+
+extern "C" int pwh_ham_setup(pwh_ham** out, const double lattice[9], const double kpt[3], const int32_t fft_dims[3],
+                             int64_t npw, const int32_t* gvec, const double* vloc, int64_t nproj, const pwh_c128* proj,
+                             int64_t ldp, const double* dij, void* stream) {
+  if (!out) return fail(PWH_EINVAL, "out is null");
+  *out = nullptr;
+  if (!lattice || !kpt || !fft_dims || !gvec || !vloc) return fail(PWH_EINVAL, "null argument");
+  if (npw < 1 || npw > (int64_t)INT32_MAX / 2) return fail(PWH_EINVAL, "npw = %lld out of range", (long long)npw);
+  if (nproj < 0 || nproj > (int64_t)INT32_MAX / 2) return fail(PWH_EINVAL, "nproj out of range");
+  if (nproj > 0 && (!proj || !dij)) return fail(PWH_EINVAL, "proj / dij null with nproj > 0");
+  if (nproj > 0 && ldp < npw) return fail(PWH_EINVAL, "ldp < npw");
+  if ((int64_t)fft_dims[0] * fft_dims[1] * fft_dims[2] < npw) return fail(PWH_EINVAL, "more plane waves than box points");
+  pwh_ham* h = new (std::nothrow) pwh_ham();
+  if (!h) return fail(PWH_ENOMEM, "out of host memory");
+  const int rc = setup_impl(h, lattice, kpt, fft_dims, npw, gvec, vloc, nproj, proj, ldp, dij, (cudaStream_t)stream);
+  if (rc != PWH_OK) {
+    pwh_ham_destroy(h);
+    return rc;
+  }
+  *out = h;
+  return PWH_OK;
+}
+
+extern "C" int pwh_ham_info(const pwh_ham* h, int64_t info[8]) {
+  if (!h || !info) return fail(PWH_EINVAL, "null argument");
+  info[0] = h->npw; info[1] = h->nproj; info[2] = h->n1; info[3] = h->n2; info[4] = h->n3;
+  info[5] = h->lp.ncols; info[6] = h->lp.nxl; info[7] = h->band_group;
+  return PWH_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// workspace
+// ---------------------------------------------------------------------------------------------------------------
+struct WsLayout {
+  size_t colbuf, cmat, part, y1, y2, total;
+  int64_t ldw;
+  int group;
+};
+
+static WsLayout ws_layout(const pwh_ham* h, int64_t nband) {
+  WsLayout w;
+  w.group = (int)std::min<int64_t>(h->band_group, std::max<int64_t>(nband, 1));
+  w.ldw = (int64_t)align_up((size_t)h->npw, 16);
+  size_t off = 0;
+  w.colbuf = off; off += align_up((size_t)w.group * h->n3 * h->lp.ncols_pad * sizeof(c128), 256);
+  w.cmat = off;   off += align_up((size_t)std::max<int64_t>(h->nproj, 1) * nband * sizeof(c128), 256);
+  w.part = off;   off += align_up(h->nproj > 0 ? zgemm_cn_workspace(h->nproj, nband, h->npw) : 16, 256);
+  w.y1 = off;     off += align_up((size_t)w.ldw * nband * sizeof(c128), 256);
+  w.y2 = off;     off += align_up((size_t)w.ldw * nband * sizeof(c128), 256);
+  w.total = off;
+  return w;
+}
+
+extern "C" size_t pwh_workspace_bytes(const pwh_ham* h, int64_t nband_max) {
+  if (!h || nband_max < 0) return 0;
+  return ws_layout(h, std::max<int64_t>(nband_max, 1)).total;
+}
+
+// out = alpha * ((H - c) y) - beta * yprev   for nband bands
+static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c128* yprev, int64_t ldprev, c128* out,
+                  int64_t ldout, double alpha, double cshift, double beta, unsigned char* ws, const WsLayout& w,
+                  cudaStream_t st) {
+  c128* colbuf = reinterpret_cast<c128*>(ws + w.colbuf);
+  c128* cmat = reinterpret_cast<c128*>(ws + w.cmat);
+  if (h->nproj > 0)
+    launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, y, ldy, h->dij, cmat, h->nproj, ws + w.part, st);
+  for (int64_t b0 = 0; b0 < nband; b0 += w.group) {
+    const int nb = (int)std::min<int64_t>(w.group, nband - b0);
+    launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, colbuf, nb, st);
+    launch_plane(h->lp, colbuf, nb, st);
+    launch_zfwd_gather(h->lp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                       out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+  }
+  if (h->nproj > 0)
+    launch_zgemm_nn_acc(h->npw, nband, h->nproj, alpha, h->proj, h->ldp, cmat, h->nproj, out, ldout, st);
+  CUDA_TRY(cudaGetLastError());
+  return PWH_OK;
+}
+
+static int check_ws(const pwh_ham* h, int64_t nband, void* ws, size_t ws_bytes) {
+  if (!ws) return fail(PWH_EINVAL, "workspace is null");
+  if ((uintptr_t)ws % 256 != 0) return fail(PWH_EINVAL, "workspace must be 256-byte aligned");
+  const size_t need = ws_layout(h, nband).total;
+  if (ws_bytes < need) return fail(PWH_EINVAL, "workspace too small: %zu < %zu bytes", ws_bytes, need);
+  return PWH_OK;
+}
+
+extern "C" int pwh_apply_h(pwh_ham* h, int64_t nband, const pwh_c128* psi, int64_t ldpsi, pwh_c128* hpsi, int64_t ldh,
+                           void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (nband == 0) return PWH_OK;
+  if (!psi || !hpsi) return fail(PWH_EINVAL, "psi / hpsi null");
+  if (ldpsi < h->npw || ldh < h->npw) return fail(PWH_EINVAL, "leading dimension smaller than npw");
+  int rc = check_ws(h, nband, ws, ws_bytes);
+  if (rc) return rc;
+  const WsLayout w = ws_layout(h, nband);
+  return h_step(h, nband, reinterpret_cast<const c128*>(psi), ldpsi, nullptr, 0, reinterpret_cast<c128*>(hpsi), ldh, 1.0,
+                0.0, 0.0, reinterpret_cast<unsigned char*>(ws), w, (cudaStream_t)stream);
+}
+
+extern "C" int pwh_cheb_filter(pwh_ham* h, int64_t nband, pwh_c128* psi, int64_t ld, int degree, double a, double b,
+                               double a0, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (degree < 0) return fail(PWH_EINVAL, "degree < 0");
+  if (!(b > a)) return fail(PWH_EINVAL, "need b > a");
+  if (!(a0 < a)) return fail(PWH_EINVAL, "need a0 < a");
+  if (nband == 0 || degree == 0) return PWH_OK;
+  if (!psi) return fail(PWH_EINVAL, "psi null");
+  if (ld < h->npw) return fail(PWH_EINVAL, "ld < npw");
+  int rc = check_ws(h, nband, ws, ws_bytes);
+  if (rc) return rc;
+  const WsLayout w = ws_layout(h, nband);
+  unsigned char* wsb = reinterpret_cast<unsigned char*>(ws);
+  cudaStream_t st = (cudaStream_t)stream;
+  c128* buf[3] = {reinterpret_cast<c128*>(psi), reinterpret_cast<c128*>(wsb + w.y1), reinterpret_cast<c128*>(wsb + w.y2)};
+  const int64_t lds[3] = {ld, w.ldw, w.ldw};
+  const double e = 0.5 * (b - a), c = 0.5 * (b + a), sigma1 = e / (a0 - c);
+  double sigma = sigma1;
+  // Y_1 = (sigma_1/e) (H - c) Y_0
+  rc = h_step(h, nband, buf[0], lds[0], nullptr, 0, buf[1], lds[1], sigma1 / e, c, 0.0, wsb, w, st);
+  if (rc) return rc;
+  for (int j = 1; j < degree; ++j) {
+    const double sigma_new = 1.0 / (2.0 / sigma1 - sigma);
+    const int ip = (j - 1) % 3, ic = j % 3, io = (j + 1) % 3;
+    rc = h_step(h, nband, buf[ic], lds[ic], buf[ip], lds[ip], buf[io], lds[io], 2.0 * sigma_new / e, c,
+                sigma * sigma_new, wsb, w, st);
+    if (rc) return rc;
+    sigma = sigma_new;
+  }
+  const int fin = degree % 3;
+  if (fin != 0)
+    CUDA_TRY(cudaMemcpy2DAsync(psi, (size_t)ld * sizeof(c128), buf[fin], (size_t)lds[fin] * sizeof(c128),
+                               (size_t)h->npw * sizeof(c128), (size_t)nband, cudaMemcpyDeviceToDevice, st));
+  return PWH_OK;
+}
+
+extern "C" size_t pwh_gram_workspace_bytes(int64_t npw, int64_t nx, int64_t ny) {
+  if (npw < 1 || nx < 1 || ny < 1) return 256;
+  return align_up(zgemm_cn_workspace(nx, ny, npw), 256);
+}
+
+extern "C" int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny, const pwh_c128* Y,
+                        int64_t ldy, pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream) {
+  if (npw < 1 || nx < 0 || ny < 0) return fail(PWH_EINVAL, "bad sizes");
+  if (nx == 0 || ny == 0) return PWH_OK;
+  if (nx > INT32_MAX / 2 || ny > INT32_MAX / 2) return fail(PWH_EINVAL, "nx / ny too large");
+  if (!X || !Y || !G) return fail(PWH_EINVAL, "null argument");
+  if (ldx < npw || ldy < npw || ldg < nx) return fail(PWH_EINVAL, "leading dimension too small");
+  if (!ws || (uintptr_t)ws % 256 != 0) return fail(PWH_EINVAL, "workspace null or not 256-byte aligned");
+  if (ws_bytes < pwh_gram_workspace_bytes(npw, nx, ny)) return fail(PWH_EINVAL, "workspace too small");
+  CUDA_TRY(zgemm_init());
+  launch_zgemm_cn(nx, ny, npw, reinterpret_cast<const c128*>(X), ldx, reinterpret_cast<const c128*>(Y), ldy, nullptr,
+                  reinterpret_cast<c128*>(G), ldg, ws, (cudaStream_t)stream);
+  CUDA_TRY(cudaGetLastError());
+  return PWH_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// host-buffer entry points
+// ---------------------------------------------------------------------------------------------------------------
+static int ensure(void** p, size_t* have, size_t need) {
+  if (*have >= need) return PWH_OK;
+  if (*p) cudaFree(*p);
+  *p = nullptr;
+  *have = 0;
+  CUDA_TRY(cudaMalloc(p, need));
+  *have = need;
+  return PWH_OK;
+}
+
+extern "C" int pwh_apply_h_host(pwh_ham* h, int64_t nband, const pwh_c128* psi_host, int64_t ldpsi, pwh_c128* hpsi_host,
+                                int64_t ldh, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (nband == 0) return PWH_OK;
+  if (!psi_host || !hpsi_host) return fail(PWH_EINVAL, "null argument");
+  if (ldpsi < h->npw || ldh < h->npw) return fail(PWH_EINVAL, "leading dimension smaller than npw");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t blk = (size_t)h->npw * nband * sizeof(c128), row = (size_t)h->npw * sizeof(c128);
+  int rc;
+  if ((rc = ensure(&h->st_psi, &h->st_psi_bytes, blk))) return rc;
+  if ((rc = ensure(&h->st_hpsi, &h->st_hpsi_bytes, blk))) return rc;
+  if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, pwh_workspace_bytes(h, nband)))) return rc;
+  CUDA_TRY(cudaMemcpy2DAsync(h->st_psi, row, psi_host, (size_t)ldpsi * sizeof(c128), row, nband, cudaMemcpyHostToDevice, st));
+  rc = pwh_apply_h(h, nband, (const pwh_c128*)h->st_psi, h->npw, (pwh_c128*)h->st_hpsi, h->npw, h->st_ws, h->st_ws_bytes, st);
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpy2DAsync(hpsi_host, (size_t)ldh * sizeof(c128), h->st_hpsi, row, row, nband, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return PWH_OK;
+}
+
+static int filter_blocks(pwh_ham* h, int64_t nband, int64_t block, c128* psi_dev, int64_t ld, int degree, double a,
+                         double b, double a0, cudaStream_t st) {
+  if (block <= 0 || block > nband) block = nband;
+  for (int64_t b0 = 0; b0 < nband; b0 += block) {
+    const int64_t nb = std::min(block, nband - b0);
+    int rc = pwh_cheb_filter(h, nb, (pwh_c128*)(psi_dev + b0 * ld), ld, degree, a, b, a0, h->st_ws, h->st_ws_bytes, st);
+    if (rc) return rc;
+  }
+  return PWH_OK;
+}
+
+extern "C" int pwh_cheb_filter_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
+                                    double a, double b, double a0, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (degree < 0 || !(b > a) || !(a0 < a)) return fail(PWH_EINVAL, "bad filter parameters");
+  if (nband == 0) return PWH_OK;
+  if (!psi_host) return fail(PWH_EINVAL, "psi null");
+  if (ld < h->npw) return fail(PWH_EINVAL, "ld < npw");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (block <= 0 || block > nband) block = nband;
+  const size_t blk = (size_t)h->npw * nband * sizeof(c128), row = (size_t)h->npw * sizeof(c128);
+  int rc;
+  if ((rc = ensure(&h->st_psi, &h->st_psi_bytes, blk))) return rc;
+  if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, pwh_workspace_bytes(h, block)))) return rc;
+  CUDA_TRY(cudaMemcpy2DAsync(h->st_psi, row, psi_host, (size_t)ld * sizeof(c128), row, nband, cudaMemcpyHostToDevice, st));
+  if ((rc = filter_blocks(h, nband, block, (c128*)h->st_psi, h->npw, degree, a, b, a0, st))) return rc;
+  CUDA_TRY(cudaMemcpy2DAsync(psi_host, (size_t)ld * sizeof(c128), h->st_psi, row, row, nband, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return PWH_OK;
+}
+
+extern "C" int pwh_sweep_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
+                              double a, double b, double a0, pwh_c128* hpsi_host, int64_t ldh, pwh_c128* G_host,
+                              int64_t ldg, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (degree < 0 || !(b > a) || !(a0 < a)) return fail(PWH_EINVAL, "bad filter parameters");
+  if (nband == 0) return PWH_OK;
+  if (!psi_host || !G_host) return fail(PWH_EINVAL, "null argument");
+  if (ld < h->npw || ldg < nband || (hpsi_host && ldh < h->npw)) return fail(PWH_EINVAL, "leading dimension too small");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (block <= 0 || block > nband) block = nband;
+  const size_t blk = (size_t)h->npw * nband * sizeof(c128), row = (size_t)h->npw * sizeof(c128);
+  const size_t gbytes = (size_t)nband * nband * sizeof(c128);
+  const size_t wsb = std::max(pwh_workspace_bytes(h, block), pwh_gram_workspace_bytes(h->npw, nband, nband));
+  int rc;
+  if ((rc = ensure(&h->st_psi, &h->st_psi_bytes, blk))) return rc;
+  if ((rc = ensure(&h->st_hpsi, &h->st_hpsi_bytes, blk))) return rc;
+  if ((rc = ensure(&h->st_g, &h->st_g_bytes, gbytes))) return rc;
+  if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, wsb))) return rc;
+  CUDA_TRY(cudaMemcpy2DAsync(h->st_psi, row, psi_host, (size_t)ld * sizeof(c128), row, nband, cudaMemcpyHostToDevice, st));
+  if ((rc = filter_blocks(h, nband, block, (c128*)h->st_psi, h->npw, degree, a, b, a0, st))) return rc;
+  for (int64_t b0 = 0; b0 < nband; b0 += block) {
+    const int64_t nb = std::min(block, nband - b0);
+    rc = pwh_apply_h(h, nb, (const pwh_c128*)((c128*)h->st_psi + b0 * h->npw), h->npw,
+                     (pwh_c128*)((c128*)h->st_hpsi + b0 * h->npw), h->npw, h->st_ws, h->st_ws_bytes, st);
+    if (rc) return rc;
+  }
+  rc = pwh_gram(h->npw, nband, (const pwh_c128*)h->st_psi, h->npw, nband, (const pwh_c128*)h->st_hpsi, h->npw,
+                (pwh_c128*)h->st_g, nband, h->st_ws, h->st_ws_bytes, st);
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpy2DAsync(psi_host, (size_t)ld * sizeof(c128), h->st_psi, row, row, nband, cudaMemcpyDeviceToHost, st));
+  if (hpsi_host)
+    CUDA_TRY(cudaMemcpy2DAsync(hpsi_host, (size_t)ldh * sizeof(c128), h->st_hpsi, row, row, nband, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpy2DAsync(G_host, (size_t)ldg * sizeof(c128), h->st_g, (size_t)nband * sizeof(c128),
+                             (size_t)nband * sizeof(c128), nband, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return PWH_OK;
+}
+
+extern "C" int64_t pwh_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+extern "C" const char* pwh_last_error(void) { return g_err.c_str(); }

@@ -1,0 +1,260 @@
+// zgemm.cu -- complex-FP64 GEMMs on the FP64 tensor pipe (DMMA, mma.sync.m8n8k4.f64) for the dense contractions
+// of the path:
+//   "CN":  C = A^H B   with K = npw   -> projector coefficients <p_i|psi_b> and the
+//                                        Rayleigh-Ritz Gram product Psi^H (H Psi), split over K
+//   "NN":  C += alpha A B with K = nproj -> P . (D . P^H psi) accumulated onto the recurrence term
+// tcgen05 has no f64 kind, so FP64 contractions on sm_100a are warp-level DMMA with register accumulators
+// (measured on B200: DMMA.8x8x4 peak 37.1 TFLOP/s == DFMA peak).  One complex product is four real DMMAs on
+// split re/im fragments; operands are staged gmem -> smem with a 4-stage cp.async pipeline in padded layouts
+// that make every 16-byte fragment load conflict-free.
+#include "launch.h"
+
+namespace pwh {
+
+namespace {
+
+constexpr int BM = 128, BN = 64, BK = 8, STAGES = 4, NT = 256;
+constexpr int WARPS_M = 4, WARPS_N = 2;               // 8 warps, warp tile 32 x 32 complex
+constexpr int KROW = BK * 16 + 64;                     // bytes per row of a K-major tile (== 64 mod 128)
+constexpr int MROW = BM * 16 + 32;                     // bytes per k-row of an M-major A tile (== 32 mod 128)
+constexpr int A_BYTES_K = BM * KROW;                   // 24576
+constexpr int A_BYTES_M = BK * MROW;                   // 16640
+constexpr int B_BYTES = BN * KROW;                     // 12288
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+      : "+d"(c0), "+d"(c1)
+      : "d"(a), "d"(b));
+}
+__device__ __forceinline__ double2 lds128(uint32_t addr) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+  return v;
+}
+
+enum { EPI_PARTIAL = 0, EPI_ACC = 1 };
+
+// A_KMAJOR = true : op(A)[m,k] = conj(A[k + m*lda])  (CN);   false : op(A)[m,k] = A[m + k*lda]  (NN)
+template <bool A_KMAJOR, int EPI>
+__global__ void __launch_bounds__(NT, 1)
+k_zgemm(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* __restrict__ A, int64_t lda,
+        const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  constexpr int A_BYTES = A_KMAJOR ? A_BYTES_K : A_BYTES_M;
+  constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp % WARPS_M, wn = warp / WARPS_M;
+  // CN: m-tile fastest (all tiles of one K split are co-resident and share the streamed K range through L2)
+  // NN: n-tile fastest (the CTAs that share one slab of A rows run together)
+  int tm, tn;
+  if (A_KMAJOR) { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
+  else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
+  const int m0 = tm * BM, n0 = tn * BN;
+  const int split = blockIdx.y;
+  const int64_t kbeg = (int64_t)split * k_per_split;
+  const int64_t kend = (kbeg + k_per_split < K) ? kbeg + k_per_split : K;
+  const int nkt = (int)((kend - kbeg + BK - 1) / BK);
+
+  auto load_stage = [&](int stage, int kt) {
+    const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+    const int64_t k0 = kbeg + (int64_t)kt * BK;
+    if (A_KMAJOR) {
+#pragma unroll
+      for (int i = 0; i < (BM * BK) / NT; ++i) {
+        const int idx = tid + i * NT, r = idx / BK, kk = idx % BK;
+        const bool ok = (m0 + r < M) && (k0 + kk < kend);
+        const c128* src = ok ? A + (int64_t)(m0 + r) * lda + k0 + kk : A;
+        cp_async16(sa + r * KROW + kk * 16, src, ok ? 16 : 0);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < (BM * BK) / NT; ++i) {
+        const int idx = tid + i * NT, kk = idx / BM, r = idx % BM;
+        const bool ok = (m0 + r < M) && (k0 + kk < kend);
+        const c128* src = ok ? A + (int64_t)(k0 + kk) * lda + m0 + r : A;
+        cp_async16(sa + kk * MROW + r * 16, src, ok ? 16 : 0);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < (BN * BK) / NT; ++i) {
+      const int idx = tid + i * NT, r = idx / BK, kk = idx % BK;
+      const bool ok = (n0 + r < N) && (k0 + kk < kend);
+      const c128* src = ok ? B + (int64_t)(n0 + r) * ldb + k0 + kk : B;
+      cp_async16(sb + r * KROW + kk * 16, src, ok ? 16 : 0);
+    }
+  };
+
+  double cr[4][4][2], ci[4][4][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { cr[i][j][0] = cr[i][j][1] = 0.0; ci[i][j][0] = ci[i][j][1] = 0.0; }
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; ++s) {
+    if (s < nkt) load_stage(s, s);
+    cp_async_commit();
+  }
+
+  const int frow = lane >> 2, fk = lane & 3;
+  // per-thread fragment base offsets inside a stage
+  const uint32_t a_off = A_KMAJOR ? (uint32_t)((wm * 32 + frow) * KROW + fk * 16)
+                                  : (uint32_t)(fk * MROW + (wm * 32 + frow) * 16);
+  const uint32_t b_off = (uint32_t)(A_BYTES + (wn * 32 + frow) * KROW + fk * 16);
+
+  for (int kt = 0; kt < nkt; ++kt) {
+    cp_async_wait<STAGES - 2>();
+    __syncthreads();
+    {
+      const int nk = kt + STAGES - 1;
+      if (nk < nkt) load_stage(nk % STAGES, nk);
+      cp_async_commit();
+    }
+    const uint32_t st = smem_base + (kt % STAGES) * STAGE_BYTES;
+#pragma unroll
+    for (int k4 = 0; k4 < BK / 4; ++k4) {
+      double2 a[4], b[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const uint32_t ao = A_KMAJOR ? (uint32_t)(i * 8 * KROW + k4 * 64) : (uint32_t)(k4 * 4 * MROW + i * 8 * 16);
+        a[i] = lds128(st + a_off + ao);
+        b[i] = lds128(st + b_off + (uint32_t)(i * 8 * KROW + k4 * 64));
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const double nai = -a[i].y;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (A_KMAJOR) {  // conj(a) * b
+            dmma(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
+            dmma(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
+            dmma(cr[i][j][0], cr[i][j][1], a[i].y, b[j].y);
+            dmma(ci[i][j][0], ci[i][j][1], nai, b[j].x);
+          } else {         // a * b
+            dmma(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
+            dmma(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
+            dmma(cr[i][j][0], cr[i][j][1], nai, b[j].y);
+            dmma(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
+          }
+        }
+      }
+    }
+  }
+  cp_async_wait<0>();
+
+  // epilogue: thread holds C[m = frow][n = 2*fk + {0,1}] of every 8x8 block
+  c128* Cout = C;
+  if (EPI == EPI_PARTIAL) Cout += (int64_t)split * ldc * N;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int m = m0 + wm * 32 + i * 8 + frow;
+    if (m >= M) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int n = n0 + wn * 32 + j * 8 + 2 * fk + h;
+        if (n >= N) continue;
+        c128* p = Cout + (int64_t)n * ldc + m;
+        if (EPI == EPI_PARTIAL) {
+          *p = cmake(cr[i][j][h], ci[i][j][h]);
+        } else {
+          c128 t = *p;
+          t.x = fma(alpha, cr[i][j][h], t.x);
+          t.y = fma(alpha, ci[i][j][h], t.y);
+          *p = t;
+        }
+      }
+    }
+  }
+}
+
+// C[m + n*ldc] = scale[m] * sum_s part[s][m + n*M]   (fixed summation order => deterministic)
+__global__ void __launch_bounds__(256) k_splitk_reduce(int M, int N, int nsplit, const c128* __restrict__ part,
+                                                       const double* __restrict__ scale, c128* __restrict__ C,
+                                                       int64_t ldc) {
+  const int64_t total = (int64_t)M * N;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int m = (int)(i % M);
+    const int64_t n = i / M;
+    double sx = 0.0, sy = 0.0;
+    for (int s = 0; s < nsplit; ++s) {
+      const c128 v = part[(int64_t)s * total + i];
+      sx += v.x;
+      sy += v.y;
+    }
+    const double f = scale ? scale[m] : 1.0;
+    C[n * ldc + m] = cmake(f * sx, f * sy);
+  }
+}
+
+constexpr int smem_cn() { return STAGES * (A_BYTES_K + B_BYTES); }
+constexpr int smem_nn() { return STAGES * (A_BYTES_M + B_BYTES); }
+constexpr int NUM_SMS = 148;
+
+}  // namespace
+
+cudaError_t zgemm_init() {
+  cudaError_t e = cudaFuncSetAttribute(k_zgemm<true, EPI_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_cn());
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_zgemm<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
+}
+
+int zgemm_cn_splits(int64_t M, int64_t N, int64_t K) {
+  const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
+  const int64_t max_split = (K + 4 * BK - 1) / (4 * BK);  // at least 4 k-slabs per split
+  int best = 1;
+  double best_eff = 0.0;
+  for (int waves = 1; waves <= 4; ++waves) {
+    int64_t s = (int64_t)NUM_SMS * waves / tiles;
+    if (s < 1) s = 1;
+    if (s > max_split) s = max_split;
+    const int64_t ctas = tiles * s;
+    const int64_t w = (ctas + NUM_SMS - 1) / NUM_SMS;
+    const double eff = (double)ctas / (double)(w * NUM_SMS);
+    if (eff > best_eff + 0.02) { best_eff = eff; best = (int)s; }
+  }
+  return best;
+}
+
+size_t zgemm_cn_workspace(int64_t M, int64_t N, int64_t K) {
+  return sizeof(c128) * (size_t)zgemm_cn_splits(M, N, K) * (size_t)M * (size_t)N;
+}
+
+void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda, const c128* B, int64_t ldb,
+                     const double* scale, c128* C, int64_t ldc, void* ws, cudaStream_t st) {
+  if (M <= 0 || N <= 0) return;
+  const int nsplit = zgemm_cn_splits(M, N, K);
+  const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
+  int64_t kps = (K + nsplit - 1) / nsplit;
+  kps = (kps + BK - 1) / BK * BK;
+  dim3 grid(tiles_m * tiles_n, nsplit);
+  c128* part = reinterpret_cast<c128*>(ws);
+  k_zgemm<true, EPI_PARTIAL><<<grid, NT, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
+  count_launch();
+  const int64_t total = M * N;
+  int blocks = (int)((total + 255) / 256);
+  if (blocks > NUM_SMS * 8) blocks = NUM_SMS * 8;
+  k_splitk_reduce<<<blocks, 256, 0, st>>>((int)M, (int)N, nsplit, part, scale, C, ldc);
+  count_launch();
+}
+
+void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c128* A, int64_t lda, const c128* B,
+                         int64_t ldb, c128* C, int64_t ldc, cudaStream_t st) {
+  if (M <= 0 || N <= 0 || K <= 0) return;
+  const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
+  dim3 grid(tiles_m * tiles_n, 1);
+  k_zgemm<false, EPI_ACC><<<grid, NT, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
+  count_launch();
+}
+
+}  // namespace pwh

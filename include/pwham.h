@@ -126,6 +126,32 @@ int pwh_sweep_host(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi_hos
 /* Number of kernel launches issued by this library since load (all handles, all threads). */
 int64_t pwh_launch_count(void);
 
+/*
+ * Per-kernel timing for the roofline report.  Between pwh_profile_begin() and
+ * pwh_profile_end() every kernel launch of the library is bracketed by a cudaEvent pair on its stream.
+ * pwh_profile_end synchronises the device and returns, per stage, the summed kernel time in milliseconds and the
+ * number of launches (HOST arrays of PWH_NSTAGES entries).  Not thread-safe against concurrent compute calls.
+ */
+enum {
+  PWH_STAGE_SCATTER_ZINV = 0, /* a1-a2: sphere -> z-columns, inverse z transform */
+  PWH_STAGE_PLANE = 1,        /* a3-a5: per-plane inverse y,x, V_loc multiply, forward x,y */
+  PWH_STAGE_ZFWD_GATHER = 2,  /* a6 + a9: forward z transform, gather, kinetic + recurrence epilogue */
+  PWH_STAGE_ZGEMM_CN = 3,     /* a7, a10: A^H B DMMA ZGEMM partial products (projector coefficients, Gram) */
+  PWH_STAGE_SPLITK = 4,       /* a7, a10: fixed-order split-K sum (+ D scaling) */
+  PWH_STAGE_ZGEMM_NN = 5,     /* a8: P (D C) accumulated onto the recurrence term */
+  PWH_NSTAGES = 8
+};
+int pwh_profile_begin(void);
+int pwh_profile_end(double ms[PWH_NSTAGES], int64_t launches[PWH_NSTAGES]);
+
+/*
+ * Attainable FP64 tensor-pipe (DMMA) rate of the current device at its current clocks, in TFLOP/s: a
+ * register-resident loop of `iters` x 32 independent mma.m8n8k4.f64 per warp on 2 CTAs per SM, timed with CUDA
+ * events (one warm-up launch).  It is the measured denominator for the ZGEMM roofline fraction; it touches no
+ * memory and is not part of the path.  tflops is a HOST pointer.  Synchronises `stream`.
+ */
+int pwh_probe_fp64_tensor_peak(int iters, double* tflops, void* stream);
+
 /* Introspection: fills info[0..7] = {npw, nproj, n1, n2, n3, n_zcolumns, n_xlines, reserved}. */
 int pwh_ham_info(const pwh_ham* ham, int64_t info[8]);
 

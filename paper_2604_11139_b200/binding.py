@@ -22,7 +22,10 @@ LIB_PATH = os.path.join(_HERE, "libpwham.so")
 
 EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply_h", "pwh_cheb_filter",
            "pwh_gram_workspace_bytes", "pwh_gram", "pwh_apply_h_host", "pwh_cheb_filter_host", "pwh_sweep_host",
-           "pwh_launch_count", "pwh_ham_info", "pwh_last_error"]
+           "pwh_launch_count", "pwh_ham_info", "pwh_last_error", "pwh_profile_begin", "pwh_profile_end",
+           "pwh_probe_fp64_tensor_peak"]
+
+STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "reserved6", "reserved7"]
 
 _lib = None
 
@@ -65,6 +68,12 @@ def load_library() -> ctypes.CDLL:
     L.pwh_launch_count.restype = i64
     L.pwh_ham_info.argtypes = [vp, vp]
     L.pwh_ham_info.restype = i32
+    L.pwh_profile_begin.argtypes = []
+    L.pwh_profile_begin.restype = i32
+    L.pwh_profile_end.argtypes = [vp, vp]
+    L.pwh_profile_end.restype = i32
+    L.pwh_probe_fp64_tensor_peak.argtypes = [i32, vp, vp]
+    L.pwh_probe_fp64_tensor_peak.restype = i32
     L.pwh_last_error.argtypes = []
     L.pwh_last_error.restype = ctypes.c_char_p
     _lib = L
@@ -282,3 +291,24 @@ def sweep_host(ham: Ham, psi_host, degree: int, a: float, b: float, a0: float, g
 
 def launch_count() -> int:
     return int(load_library().pwh_launch_count())
+
+
+def profile_begin() -> None:
+    _check(load_library().pwh_profile_begin(), "pwh_profile_begin")
+
+
+def profile_end() -> dict:
+    """Returns {stage: (milliseconds, launches)} summed over the launches since profile_begin()."""
+    ms = (ctypes.c_double * 8)()
+    n = (ctypes.c_int64 * 8)()
+    _check(load_library().pwh_profile_end(ms, n), "pwh_profile_end")
+    return {STAGES[i]: (float(ms[i]), int(n[i])) for i in range(8) if n[i]}
+
+
+def probe_fp64_tensor_peak(iters: int = 20000, device="cuda:0") -> float:
+    """TFLOP/s of a register-resident DMMA loop on this GPU at its current clocks (roofline denominator)."""
+    out = ctypes.c_double(0.0)
+    with torch.cuda.device(device):
+        _check(load_library().pwh_probe_fp64_tensor_peak(int(iters), ctypes.byref(out), _stream_ptr(torch.device(device))),
+               "pwh_probe_fp64_tensor_peak")
+    return float(out.value)

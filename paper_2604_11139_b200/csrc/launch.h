@@ -6,6 +6,18 @@ namespace pwh {
 
 void count_launch();
 
+// Stage ids reported by pwh_profile_end (same order as PWH_STAGE_* in include/pwham.h).
+enum { ST_SCATTER_ZINV = 0, ST_PLANE = 1, ST_ZFWD_GATHER = 2, ST_ZGEMM_CN = 3, ST_SPLITK = 4, ST_ZGEMM_NN = 5 };
+// Counts one kernel launch and, while profiling is on, brackets it with a cudaEvent pair on `st`.
+class ScopedLaunch {
+ public:
+  ScopedLaunch(int stage, cudaStream_t st);
+  ~ScopedLaunch();
+ private:
+  cudaStream_t st_;
+  int64_t idx_;
+};
+
 // local_kernels.cu
 size_t zkernel_smem(const LocalPlan& P);
 size_t plane_smem(const LocalPlan& P);
@@ -18,6 +30,8 @@ void launch_zfwd_gather(const LocalPlan& P, const c128* colbuf, const c128* y, i
 
 // zgemm.cu
 cudaError_t zgemm_init();
+// runs `ctas` CTAs x 8 warps x iters x 32 DMMA.8x8x4 (512 flop each) and returns the elapsed milliseconds
+cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float* ms);
 // number of K splits chosen for C(M x N) = A^H B with K = npw
 int zgemm_cn_splits(int64_t M, int64_t N, int64_t K);
 size_t zgemm_cn_workspace(int64_t M, int64_t N, int64_t K);

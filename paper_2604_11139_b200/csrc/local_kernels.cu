@@ -161,22 +161,22 @@ cudaError_t local_kernels_init(const LocalPlan& P) {
 
 void launch_scatter_zinv(const LocalPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st) {
   dim3 grid(P.ngrp, nb);
+  ScopedLaunch sl(ST_SCATTER_ZINV, st);
   k_scatter_zinv<<<grid, ZT, zkernel_smem(P), st>>>(P, psi, ldpsi, colbuf);
-  count_launch();
 }
 
 void launch_plane(const LocalPlan& P, c128* colbuf, int nb, cudaStream_t st) {
   dim3 grid(P.n3, nb);
+  ScopedLaunch sl(ST_PLANE, st);
   k_plane<<<grid, PT, plane_smem(P), st>>>(P, colbuf);
-  count_launch();
 }
 
 void launch_zfwd_gather(const LocalPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,
                         int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
                         cudaStream_t st) {
   dim3 grid(P.ngrp, nb);
+  ScopedLaunch sl(ST_ZFWD_GATHER, st);
   k_zfwd_gather<<<grid, ZT, zkernel_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha, cshift, beta);
-  count_launch();
 }
 
 }  // namespace pwh

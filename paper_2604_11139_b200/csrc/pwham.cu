@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -20,6 +21,35 @@ using namespace pwh;
 namespace pwh {
 static std::atomic<int64_t> g_launches{0};
 void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+// Optional per-launch timing (pwh_profile_begin / pwh_profile_end): one cudaEvent pair around every kernel launch,
+// recorded on the launching stream.  Off by default; the hot path then pays one relaxed atomic load per launch.
+struct ProfRec { int stage; cudaEvent_t e0, e1; };
+static std::atomic<bool> g_prof_on{false};
+static std::mutex g_prof_mu;
+static std::vector<ProfRec> g_prof;
+static std::vector<cudaEvent_t> g_prof_pool;
+
+static cudaEvent_t prof_event() {
+  cudaEvent_t e = nullptr;
+  if (!g_prof_pool.empty()) { e = g_prof_pool.back(); g_prof_pool.pop_back(); }
+  else cudaEventCreate(&e);
+  return e;
+}
+ScopedLaunch::ScopedLaunch(int stage, cudaStream_t st) : st_(st), idx_(-1) {
+  count_launch();
+  if (!g_prof_on.load(std::memory_order_relaxed)) return;
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  ProfRec r{stage, prof_event(), prof_event()};
+  cudaEventRecord(r.e0, st_);
+  idx_ = (int64_t)g_prof.size();
+  g_prof.push_back(r);
+}
+ScopedLaunch::~ScopedLaunch() {
+  if (idx_ < 0) return;
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  cudaEventRecord(g_prof[(size_t)idx_].e1, st_);
+}
 }  // namespace pwh
 
 static thread_local std::string g_err;
@@ -613,6 +643,44 @@ extern "C" int pwh_sweep_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128
   CUDA_TRY(cudaMemcpy2DAsync(G_host, (size_t)ldg * sizeof(c128), h->st_g, (size_t)nband * sizeof(c128),
                              (size_t)nband * sizeof(c128), nband, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
+  return PWH_OK;
+}
+
+extern "C" int pwh_probe_fp64_tensor_peak(int iters, double* tflops, void* stream) {
+  if (!tflops || iters < 1) return fail(PWH_EINVAL, "bad arguments");
+  double* sink = nullptr;
+  CUDA_TRY(cudaMalloc(&sink, 16));
+  const int ctas = 148 * 2;
+  float ms = 0.f;
+  cudaError_t e = dmma_probe(iters, ctas, sink, (cudaStream_t)stream, &ms);
+  cudaFree(sink);
+  CUDA_TRY(e);
+  *tflops = (double)ctas * 8.0 * (double)iters * 32.0 * 512.0 / ((double)ms * 1e-3) * 1e-12;
+  return PWH_OK;
+}
+
+extern "C" int pwh_profile_begin(void) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  for (auto& r : g_prof) { g_prof_pool.push_back(r.e0); g_prof_pool.push_back(r.e1); }
+  g_prof.clear();
+  g_prof_on.store(true);
+  return PWH_OK;
+}
+
+extern "C" int pwh_profile_end(double ms[PWH_NSTAGES], int64_t launches[PWH_NSTAGES]) {
+  if (!ms || !launches) return fail(PWH_EINVAL, "null argument");
+  g_prof_on.store(false);
+  CUDA_TRY(cudaDeviceSynchronize());
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  for (int i = 0; i < PWH_NSTAGES; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  for (auto& r : g_prof) {
+    float t = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&t, r.e0, r.e1));
+    if (r.stage >= 0 && r.stage < PWH_NSTAGES) { ms[r.stage] += (double)t; launches[r.stage] += 1; }
+    g_prof_pool.push_back(r.e0);
+    g_prof_pool.push_back(r.e1);
+  }
+  g_prof.clear();
   return PWH_OK;
 }
 

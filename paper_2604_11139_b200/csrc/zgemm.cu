@@ -197,6 +197,23 @@ __global__ void __launch_bounds__(256) k_splitk_reduce(int M, int N, int nsplit,
   }
 }
 
+// Register-resident DMMA loop: the attainable FP64 tensor-pipe rate on this GPU at its current clocks (the
+// denominator of the ZGEMM roofline fraction).  32 independent accumulator pairs per warp, no memory traffic.
+__global__ void __launch_bounds__(256) k_dmma_probe(int iters, double* __restrict__ sink) {
+  double c[32][2];
+#pragma unroll
+  for (int i = 0; i < 32; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
+  double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 32; ++i) dmma(c[i][0], c[i][1], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 32; ++i) s += c[i][0] + c[i][1];
+  if (s == 12345.678) sink[0] = s;
+}
+
 constexpr int smem_cn() { return STAGES * (A_BYTES_K + B_BYTES); }
 constexpr int smem_nn() { return STAGES * (A_BYTES_M + B_BYTES); }
 constexpr int NUM_SMS = 148;
@@ -207,6 +224,24 @@ cudaError_t zgemm_init() {
   cudaError_t e = cudaFuncSetAttribute(k_zgemm<true, EPI_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_cn());
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_zgemm<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
+}
+
+cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float* ms) {
+  cudaEvent_t e0, e1;
+  cudaError_t e;
+  if ((e = cudaEventCreate(&e0)) != cudaSuccess) return e;
+  if ((e = cudaEventCreate(&e1)) != cudaSuccess) return e;
+  k_dmma_probe<<<ctas, 256, 0, st>>>(iters / 8 + 1, sink);  // warm-up
+  cudaEventRecord(e0, st);
+  k_dmma_probe<<<ctas, 256, 0, st>>>(iters, sink);
+  cudaEventRecord(e1, st);
+  count_launch();
+  count_launch();
+  e = cudaEventSynchronize(e1);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return e;
 }
 
 int zgemm_cn_splits(int64_t M, int64_t N, int64_t K) {
@@ -239,13 +274,15 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
   kps = (kps + BK - 1) / BK * BK;
   dim3 grid(tiles_m * tiles_n, nsplit);
   c128* part = reinterpret_cast<c128*>(ws);
-  k_zgemm<true, EPI_PARTIAL><<<grid, NT, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
-  count_launch();
+  {
+    ScopedLaunch sl(ST_ZGEMM_CN, st);
+    k_zgemm<true, EPI_PARTIAL><<<grid, NT, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
+  }
   const int64_t total = M * N;
   int blocks = (int)((total + 255) / 256);
   if (blocks > NUM_SMS * 8) blocks = NUM_SMS * 8;
+  ScopedLaunch sl(ST_SPLITK, st);
   k_splitk_reduce<<<blocks, 256, 0, st>>>((int)M, (int)N, nsplit, part, scale, C, ldc);
-  count_launch();
 }
 
 void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c128* A, int64_t lda, const c128* B,
@@ -253,8 +290,8 @@ void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c1
   if (M <= 0 || N <= 0 || K <= 0) return;
   const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
   dim3 grid(tiles_m * tiles_n, 1);
+  ScopedLaunch sl(ST_ZGEMM_NN, st);
   k_zgemm<false, EPI_ACC><<<grid, NT, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
-  count_launch();
 }
 
 }  // namespace pwh

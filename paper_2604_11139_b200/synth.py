@@ -242,3 +242,34 @@ def make_workload(cfg_id: int, *, with_psi: bool = True, qr: str = "numpy",
     return Workload(spec=spec, lattice=lattice, kpt=kpt, fft_dims=np.asarray(spec.fft_dims, dtype=np.int32),
                     gvec=gvec, vloc=vloc, proj=proj, dij=dij, psi=psi, atoms=atoms, depths=depths,
                     degree=spec.degree, a=a, b=b, a0=a0)
+
+
+def random_problem(dims, cell, kpt, ecut, nproj, nband, seed) -> Workload:
+    """A small unstructured orthorhombic problem for parity edge cases (odd radices, non-cubic boxes, k-shifts):
+    the plane waves with 1/2|k+G|^2 <= ecut, random V_loc, random dense projectors, random (not orthonormal) Psi.
+    Inputs only; the filter bounds are crude brackets (a0 < a < b) that keep the recurrence well-conditioned."""
+    rng = np.random.default_rng(np.random.SeedSequence(list(SEED_ROOT) + [1000 + int(seed)]))
+    spec = ConfigSpec(1000 + int(seed), f"random_{dims[0]}x{dims[1]}x{dims[2]}", tuple(float(c) for c in cell),
+                      tuple(float(k) for k in kpt), tuple(int(d) for d in dims), ("ecut", float(ecut)), int(nband),
+                      int(nband), 0, "sp", (0.0, 0.0), 3, False)
+    lattice = np.diag(np.asarray(spec.cell, dtype=np.float64))
+    B = reciprocal(lattice)
+    k = np.asarray(spec.kpt, dtype=np.float64)
+    gvec = gsphere(spec)
+    npw = gvec.shape[0]
+    q = (gvec.astype(np.float64) + k[None, :]) @ B
+    kin = 0.5 * np.einsum("ij,ij->i", q, q)
+    n1, n2, n3 = spec.fft_dims
+    vloc = rng.uniform(-1.0, 1.0, size=(n3, n2, n1))
+    proj = (rng.standard_normal((nproj, npw)) + 1j * rng.standard_normal((nproj, npw))) * (0.5 / math.sqrt(npw))
+    dij = rng.uniform(-5.0, 5.0, size=nproj)
+    psi = (rng.standard_normal((nband, npw)) + 1j * rng.standard_normal((nband, npw))) / math.sqrt(2.0 * npw)
+    p2 = proj.real ** 2 + proj.imag ** 2
+    b = float(kin.max() + vloc.max() + (np.abs(dij) @ p2.sum(axis=1) if nproj else 0.0))
+    lo = float(kin.min() + vloc.min() - (np.abs(dij) @ p2.sum(axis=1) if nproj else 0.0))
+    a = lo + 0.5 * (b - lo)
+    a0 = lo - 0.05 * (b - lo)
+    return Workload(spec=spec, lattice=lattice, kpt=k, fft_dims=np.asarray(spec.fft_dims, dtype=np.int32), gvec=gvec,
+                    vloc=np.ascontiguousarray(vloc), proj=np.ascontiguousarray(proj), dij=dij,
+                    psi=np.ascontiguousarray(psi), atoms=np.zeros((0, 3)), depths=np.zeros((0,)), degree=3, a=a, b=b,
+                    a0=a0)

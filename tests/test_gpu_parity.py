@@ -1,0 +1,285 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's: relative Frobenius error 1e-11 for H.Psi and Gram
+matrices, 1e-9 for filtered blocks (complex128).  Every test here needs a B200 (`-m gpu`).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2604_11139_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_H = 1e-11
+TOL_F = 1e-9
+
+
+def relerr(x, ref):
+    return float(np.linalg.norm(np.asarray(x) - np.asarray(ref)) / max(np.linalg.norm(ref), 1e-300))
+
+
+def ham_args(w):
+    return (w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, w.proj, w.dij)
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    from paper_2604_11139_b200 import binding
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    binding.load_library()
+    return binding
+
+
+def setup(binding, w, proj="default", vloc=None):
+    p = w.proj if isinstance(proj, str) else proj
+    d = w.dij if isinstance(proj, str) else (w.dij[: 0 if proj is None else len(proj)])
+    return binding.ham_setup(w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc if vloc is None else vloc, p, d)
+
+
+def to_dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# apply_h
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2"])
+def test_apply_h_matches_oracle(gpu, cfg, request):
+    w = request.getfixturevalue(cfg)
+    ham = setup(gpu, w)
+    out = gpu.apply_h(ham, to_dev(w.psi)).cpu().numpy()
+    ref = oracle.apply_h(*ham_args(w), w.psi)
+    assert relerr(out, ref) <= TOL_H
+    # element by element, scaled by the block's largest entry
+    assert np.abs(out - ref).max() <= 1e-11 * np.abs(ref).max()
+    ham.destroy()
+
+
+@pytest.mark.parametrize("term", ["kin", "loc", "nl"])
+def test_apply_h_single_terms_cfg2(gpu, cfg2, term):
+    """Each additive term alone (kinetic, local, nonlocal), so that a large term cannot mask a small one."""
+    w = cfg2
+    psi = w.psi[:24]
+    if term == "kin":
+        ham = setup(gpu, w, proj=None, vloc=np.zeros_like(w.vloc))
+        ref = oracle.apply_h(*ham_args(w), psi, terms=oracle.TERM_KIN)
+    elif term == "loc":
+        ham = setup(gpu, w, proj=None)
+        ref = oracle.apply_h(*ham_args(w), psi, terms=oracle.TERM_KIN | oracle.TERM_LOC)
+    else:
+        ham = setup(gpu, w, vloc=np.zeros_like(w.vloc))
+        ref = oracle.apply_h(*ham_args(w), psi, terms=oracle.TERM_KIN | oracle.TERM_NL)
+    out = gpu.apply_h(ham, to_dev(psi)).cpu().numpy()
+    if term == "loc":   # subtract the (exactly diagonal) kinetic part so the local term is compared on its own scale
+        kin = oracle.kinetic(w.lattice, w.kpt, w.gvec)
+        assert relerr(out - kin[None, :] * psi, ref - kin[None, :] * psi) <= 10 * TOL_H
+    assert relerr(out, ref) <= TOL_H
+    ham.destroy()
+
+
+RANDOM_CASES = [
+    # dims,           cell,             kpt,                     ecut, nproj, nband   (radices exercised)
+    ((20, 24, 30), (8.0, 9.0, 11.0), (0.25, -0.125, 0.375), 4.0, 7, 5),     # 4*5, 8*3, 5*3*2
+    ((10, 12, 18), (5.0, 6.0, 9.0), (0.0, 0.0, 0.0), 2.5, 3, 3),            # 5*2, 4*3, 3*3*2
+    ((25, 27, 32), (9.0, 9.5, 11.0), (0.5, 0.5, 0.5), 4.0, 130, 67),        # 5*5, 3*3*3, 8*4; ragged GEMM tiles
+    ((6, 6, 6), (4.0, 4.0, 4.0), (0.1, 0.2, 0.3), 1.5, 1, 1),               # 5 plane waves, one band, one projector
+    ((64, 40, 36), (14.0, 9.0, 8.0), (0.25, 0.25, 0.25), 6.0, 0, 9),        # no projectors
+    ((2, 2, 2), (2.0, 2.0, 2.0), (0.0, 0.0, 0.0), 0.1, 2, 2),               # one plane wave, smallest box
+]
+
+
+@pytest.mark.parametrize("case", range(len(RANDOM_CASES)))
+def test_random_boxes_apply_filter_gram(gpu, case):
+    dims, cell, kpt, ecut, nproj, nband = RANDOM_CASES[case]
+    w = synth.random_problem(dims, cell, kpt, ecut, nproj, nband, seed=case)
+    ham = setup(gpu, w)
+    psi = to_dev(w.psi)
+    hpsi = gpu.apply_h(ham, psi)
+    ref_h = oracle.apply_h(*ham_args(w), w.psi)
+    assert relerr(hpsi.cpu().numpy(), ref_h) <= TOL_H
+    g = gpu.gram(psi, hpsi).cpu().numpy()
+    assert relerr(g, oracle.gram(w.psi, ref_h)) <= TOL_H
+    for m in (1, 2, 3, 5):
+        y = gpu.cheb_filter(ham, psi.clone(), m, w.a, w.b, w.a0).cpu().numpy()
+        ref = oracle.cheb_filter(*ham_args(w), w.psi, m, w.a, w.b, w.a0)
+        assert relerr(y, ref) <= TOL_F, (case, m)
+    ham.destroy()
+
+
+def test_cfg3_band_subset(gpu):
+    """Config 3 (k = 1/4 1/4 1/4, 96^3, 57925 plane waves, 512 projectors) at full N and J on a subset of bands --
+    exact, since bands never interact before gram."""
+    w = synth.make_workload(3, nband=12, qr="numpy")
+    ham = setup(gpu, w)
+    info = ham.info()
+    assert info["npw"] == synth.EXPECTED_NPW[3] and info["n_zcolumns"] == 1808 and info["n_xlines"] == 48
+    psi = to_dev(w.psi)
+    hpsi = gpu.apply_h(ham, psi)
+    ref_h = oracle.apply_h(*ham_args(w), w.psi)
+    assert relerr(hpsi.cpu().numpy(), ref_h) <= TOL_H
+    y = gpu.cheb_filter(ham, psi.clone(), 4, w.a, w.b, w.a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(w), w.psi, 4, w.a, w.b, w.a0)) <= TOL_F
+    g = gpu.gram(psi, hpsi).cpu().numpy()
+    assert relerr(g, oracle.gram(w.psi, ref_h)) <= TOL_H
+    ham.destroy()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# cheb_filter
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,degrees", [("cfg1", (0, 1, 2, 3, 4, 7, 16)), ("cfg2", (1, 8))])
+def test_cheb_filter_matches_oracle(gpu, cfg, degrees, request):
+    w = request.getfixturevalue(cfg)
+    ham = setup(gpu, w)
+    for m in degrees:
+        y = gpu.cheb_filter(ham, to_dev(w.psi), m, w.a, w.b, w.a0).cpu().numpy()
+        ref = oracle.cheb_filter(*ham_args(w), w.psi, m, w.a, w.b, w.a0)
+        assert relerr(y, ref) <= TOL_F, m
+    ham.destroy()
+
+
+def test_cheb_filter_paper_bounds_rule(gpu, cfg1):
+    """Bounds from Rayleigh quotients as in Algorithm 12 line 3: a0 = min RQ, a = max RQ."""
+    w = cfg1
+    hp = oracle.apply_h(*ham_args(w), w.psi)
+    rq = np.real(np.einsum("bg,bg->b", w.psi.conj(), hp))
+    a0, a = float(rq.min()) - 1e-3, float(rq.max())
+    ham = setup(gpu, w)
+    y = gpu.cheb_filter(ham, to_dev(w.psi), 6, a, w.b, a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(w), w.psi, 6, a, w.b, a0)) <= TOL_F
+    ham.destroy()
+
+
+def test_filter_is_m_applications_of_h(gpu, cfg1):
+    """Degree-1 filter == (sigma_1/e)(H - c) psi computed from apply_h (the recurrence's first step)."""
+    w = cfg1
+    ham = setup(gpu, w)
+    psi = to_dev(w.psi)
+    e, c = 0.5 * (w.b - w.a), 0.5 * (w.b + w.a)
+    s1 = e / (w.a0 - c)
+    y1 = gpu.cheb_filter(ham, psi.clone(), 1, w.a, w.b, w.a0)
+    manual = (s1 / e) * (gpu.apply_h(ham, psi) - c * psi)
+    assert relerr(y1.cpu().numpy(), manual.cpu().numpy()) <= 1e-13
+    ham.destroy()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# gram
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nx,ny,npw", [(1, 1, 1), (3, 5, 17), (16, 16, 257), (128, 128, 7153), (130, 67, 4099),
+                                       (64, 200, 33)])
+def test_gram_matches_oracle(gpu, nx, ny, npw):
+    rng = np.random.default_rng(nx * 1000 + ny)
+    x = (rng.standard_normal((nx, npw)) + 1j * rng.standard_normal((nx, npw)))
+    y = (rng.standard_normal((ny, npw)) + 1j * rng.standard_normal((ny, npw)))
+    g = gpu.gram(to_dev(x), to_dev(y)).cpu().numpy()
+    ref = oracle.gram(x, y)
+    assert g.shape == (nx, ny)
+    assert relerr(g, ref) <= TOL_H
+    assert np.abs(g - ref).max() <= 1e-11 * np.abs(ref).max() * math.sqrt(npw)
+
+
+def test_gram_of_orthonormal_block_and_hermiticity(gpu, cfg2):
+    w = cfg2
+    ham = setup(gpu, w)
+    psi = to_dev(w.psi)
+    s = gpu.gram(psi, psi).cpu().numpy()
+    assert np.abs(s - np.eye(w.nband)).max() <= 1e-13
+    hpsi = gpu.apply_h(ham, psi)
+    hsub = gpu.gram(psi, hpsi).cpu().numpy()
+    assert np.abs(hsub - hsub.conj().T).max() <= 1e-12 * np.abs(hsub).max()
+    assert relerr(hsub, oracle.gram(w.psi, oracle.apply_h(*ham_args(w), w.psi))) <= TOL_H
+    # deterministic: the split-K reduction has a fixed order
+    assert np.array_equal(hsub, gpu.gram(psi, hpsi).cpu().numpy())
+    ham.destroy()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# layout, ownership, errors, host entry points
+# ----------------------------------------------------------------------------------------------------------------
+def test_padded_leading_dimension_is_untouched(gpu, cfg1):
+    import torch
+    w = cfg1
+    ham = setup(gpu, w)
+    ld = w.npw + 7
+    buf = torch.full((w.nband, ld), complex(7.0, -3.0), dtype=torch.complex128, device="cuda")
+    buf[:, : w.npw] = to_dev(w.psi)
+    out = torch.full((w.nband, ld + 2), complex(1.0, 2.0), dtype=torch.complex128, device="cuda")
+    gpu.apply_h(ham, buf[:, : w.npw], out[:, : w.npw])
+    ref = oracle.apply_h(*ham_args(w), w.psi)
+    assert relerr(out[:, : w.npw].cpu().numpy(), ref) <= TOL_H
+    assert torch.all(out[:, w.npw:] == complex(1.0, 2.0))
+    gpu.cheb_filter(ham, buf[:, : w.npw], 5, w.a, w.b, w.a0)
+    assert relerr(buf[:, : w.npw].cpu().numpy(), oracle.cheb_filter(*ham_args(w), w.psi, 5, w.a, w.b, w.a0)) <= TOL_F
+    assert torch.all(buf[:, w.npw:] == complex(7.0, -3.0))
+    ham.destroy()
+
+
+def test_band_independence_and_blocking(gpu, cfg2):
+    """Filtering a block == filtering its column blocks separately (cfg 5's 'blocks of 512'), bit for bit."""
+    w = cfg2
+    ham = setup(gpu, w)
+    full = gpu.cheb_filter(ham, to_dev(w.psi), 3, w.a, w.b, w.a0)
+    parts = to_dev(w.psi)
+    for b0 in range(0, w.nband, 48):
+        gpu.cheb_filter(ham, parts[b0:b0 + 48], 3, w.a, w.b, w.a0)
+    assert relerr(parts.cpu().numpy(), full.cpu().numpy()) <= 1e-14
+    ham.destroy()
+
+
+def test_error_codes(gpu, cfg1):
+    import torch
+    w = cfg1
+    with pytest.raises(gpu.PwhamError, match="prime factors"):
+        gpu.ham_setup(w.lattice, w.kpt, (14, 16, 16), w.gvec, np.zeros((16, 16, 14)), w.proj, w.dij)
+    bad = w.gvec.copy()
+    bad[1] = bad[0] + np.array([16, 0, 0])      # wraps onto plane wave 0
+    with pytest.raises(gpu.PwhamError, match="collides"):
+        gpu.ham_setup(w.lattice, w.kpt, w.fft_dims, bad, w.vloc, w.proj, w.dij)
+    ham = setup(gpu, w)
+    psi = to_dev(w.psi)
+    with pytest.raises(gpu.PwhamError, match="b > a"):
+        gpu.cheb_filter(ham, psi, 3, 2.0, 1.0, 0.0)
+    with pytest.raises(gpu.PwhamError, match="a0 < a"):
+        gpu.cheb_filter(ham, psi, 3, 1.0, 2.0, 1.5)
+    with pytest.raises(gpu.PwhamError, match="degree"):
+        gpu.cheb_filter(ham, psi, -1, 1.0, 2.0, 0.0)
+    L = gpu.load_library()
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    rc = L.pwh_apply_h(ham.handle, w.nband, psi.data_ptr(), w.npw, psi.data_ptr(), w.npw, ws.data_ptr(), 16, None)
+    assert rc == -1 and b"workspace" in L.pwh_last_error()
+    rc = L.pwh_apply_h(ham.handle, w.nband, psi.data_ptr(), w.npw - 1, psi.data_ptr(), w.npw, ws.data_ptr(), 16, None)
+    assert rc == -1
+    assert L.pwh_apply_h(ham.handle, 0, None, 0, None, 0, None, 0, None) == 0      # nband == 0: no-op
+    ham.destroy()
+
+
+def test_host_entry_points(gpu, cfg2):
+    """The end-to-end calls bench.py times: host buffers in, host buffers out, same kernels."""
+    import torch
+    w = cfg2
+    ham = setup(gpu, w)
+    psi_h = torch.from_numpy(w.psi.copy()).pin_memory()
+    hpsi_h = torch.empty_like(psi_h).pin_memory()
+    gpu.apply_h_host(ham, psi_h, hpsi_h)
+    ref_h = oracle.apply_h(*ham_args(w), w.psi)
+    assert relerr(hpsi_h.numpy(), ref_h) <= TOL_H
+    y_h = torch.from_numpy(w.psi.copy()).pin_memory()
+    gpu.cheb_filter_host(ham, y_h, 4, w.a, w.b, w.a0, block=40)
+    ref_y = oracle.cheb_filter(*ham_args(w), w.psi, 4, w.a, w.b, w.a0)
+    assert relerr(y_h.numpy(), ref_y) <= TOL_F
+    z_h = torch.from_numpy(w.psi.copy()).pin_memory()
+    g_h = torch.empty((w.nband, w.nband), dtype=torch.complex128).pin_memory()
+    hz_h = torch.empty_like(z_h).pin_memory()
+    n0 = gpu.launch_count()
+    gpu.sweep_host(ham, z_h, 4, w.a, w.b, w.a0, g_h, block=64, hpsi_host=hz_h)
+    assert gpu.launch_count() > n0
+    assert relerr(z_h.numpy(), ref_y) <= TOL_F
+    ref_hy = oracle.apply_h(*ham_args(w), ref_y)
+    assert relerr(hz_h.numpy(), ref_hy) <= TOL_F
+    assert relerr(g_h.numpy().T, oracle.gram(ref_y, ref_hy)) <= TOL_F
+    ham.destroy()

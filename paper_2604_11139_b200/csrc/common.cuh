@@ -79,4 +79,25 @@ struct LocalPlan {
   FastDiv div_colgrp, div_nxl, div_xbatch, div_n1, div_ncols_pad;
 };
 
+// Plan of the register-resident two-pass local kernels (local_fast.cu): every axis n = r1 * r2.
+struct FastPlan {
+  int n1, n2, n3;
+  int r1[3], r2[3];          // x, y, z
+  const c128* tw[3];         // tw[ax][t] = exp(+2 pi i t / n_ax), t < n_ax
+  int ncols, ncols_pad, nxl;
+  int colgrp, ngrp;          // columns per CTA of the z kernels, number of column groups
+  int zstride, ystride;      // odd shared-memory line strides (elements)
+  int yb;                    // y-slots per x batch in the plane kernel
+  int tsize;                 // elements of the x-batch buffer T (0 when the x transform is a single pass)
+  int plane_threads;         // block size of the plane kernel
+  const int* grp_ptr;        // [ngrp+1] CSR over sphere entries sorted by column group
+  const int* ent_pw;         // [npw] plane-wave index of each entry
+  const int* ent_off;        // [npw] lcol*zstride + wrapped z
+  const int* col_hp;         // [ncols_pad] xl*ystride + wrapped y of each column
+  const short* xl_of_x;      // [n1] x-line index of each wrapped x, -1 if untouched
+  const double* vslot;       // [n3 slots][n1 slots][n2 slots] V_loc/F, y-slot fastest
+  const double* kin;         // [npw]
+  FastDiv div_colgrp, div_nxl, div_yb;
+};
+
 }  // namespace pwh

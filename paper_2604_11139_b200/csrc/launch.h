@@ -28,6 +28,16 @@ void launch_zfwd_gather(const LocalPlan& P, const c128* colbuf, const c128* y, i
                         int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
                         cudaStream_t st);
 
+// local_fast.cu
+size_t fast_zkernel_smem(const FastPlan& P);
+size_t fast_plane_smem(const FastPlan& P);
+cudaError_t fast_kernels_init(const FastPlan& P);
+void launch_fast_scatter_zinv(const FastPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st);
+void launch_fast_plane(const FastPlan& P, c128* colbuf, int nb, cudaStream_t st);
+void launch_fast_zfwd_gather(const FastPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,
+                             int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
+                             cudaStream_t st);
+
 // zgemm.cu
 cudaError_t zgemm_init();
 // runs `ctas` CTAs x 8 warps x iters x 32 DMMA.8x8x4 (512 flop each) and returns the elapsed milliseconds

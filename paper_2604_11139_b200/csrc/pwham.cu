@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -76,6 +77,8 @@ struct pwh_ham {
   int64_t npw = 0, nproj = 0;
   int n1 = 0, n2 = 0, n3 = 0;
   LocalPlan lp;
+  FastPlan fp;
+  bool fast = false;
   const c128* proj = nullptr;
   int64_t ldp = 0;
   double* dij = nullptr;
@@ -156,6 +159,36 @@ static bool make_axis_plan(int n, AxisPlan& pl, std::vector<c128>& tw, std::vect
   return true;
 }
 
+// n = r1 * r2 with r1 in {1..6,8,9,10,12,15,16}, r2 in {1..6,8,9,10,12}, r1 >= r2, |r1 - r2| minimal; n <= 16 -> r2 = 1
+static bool factor_two_pass(int n, int& r1, int& r2) {
+  static const int S1[] = {1, 2, 3, 4, 5, 6, 8, 9, 10, 12, 15, 16};
+  static const int S2[] = {1, 2, 3, 4, 5, 6, 8, 9, 10, 12};
+  auto in = [](const int* s, int len, int v) { for (int i = 0; i < len; ++i) if (s[i] == v) return true; return false; };
+  if (n <= 16 && in(S1, 12, n)) { r1 = n; r2 = 1; return true; }
+  int best = -1;
+  for (int b : S2) {
+    if (b < 2 || n % b) continue;
+    const int a = n / b;
+    if (a < b || !in(S1, 12, a)) continue;
+    if (best < 0 || a - b < best) { best = a - b; r1 = a; r2 = b; }
+  }
+  return best >= 0;
+}
+
+// V_loc/F in slot order, y-slot fastest: out[(zs*n1 + xs)*n2 + ys] = v[px(xs) + n1*(py(ys) + n2*pz(zs))] / F,
+// p(s) = s / r2 + r1 * (s % r2)
+__global__ void k_slot_vloc(int n1, int n2, int n3, int r1x, int r2x, int r1y, int r2y, int r1z, int r2z,
+                            const double* __restrict__ v, double inv_f, double* __restrict__ out) {
+  const int64_t total = (int64_t)n1 * n2 * n3;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int ys = (int)(i % n2);
+    const int xs = (int)((i / n2) % n1);
+    const int zs = (int)(i / ((int64_t)n1 * n2));
+    const int x = xs / r2x + r1x * (xs % r2x), y = ys / r2y + r1y * (ys % r2y), z = zs / r2z + r1z * (zs % r2z);
+    out[i] = v[x + (int64_t)n1 * (y + (int64_t)n2 * z)] * inv_f;
+  }
+}
+
 __global__ void k_permute_vloc(int n1, int n2, int n3, const double* __restrict__ v, const int* __restrict__ natx,
                                const int* __restrict__ naty, const int* __restrict__ natz, double inv_f,
                                double* __restrict__ out) {
@@ -208,7 +241,16 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   memset(&lp, 0, sizeof(lp));
   lp.n1 = n1; lp.n2 = n2; lp.n3 = n3;
 
-  // FFT plans
+  // FFT plans: register-resident two-pass plan when every axis factors as r1 * r2, otherwise the generic
+  // radix-2/3/4/5/8 shared-memory stages (PWH_FORCE_GENERIC_FFT=1 forces the latter; used by the tests)
+  FastPlan& fp = h->fp;
+  memset(&fp, 0, sizeof(fp));
+  {
+    const char* force = getenv("PWH_FORCE_GENERIC_FFT");
+    bool ok = !(force && force[0] == '1');
+    for (int ax = 0; ax < 3 && ok; ++ax) ok = factor_two_pass(dims[ax], fp.r1[ax], fp.r2[ax]);
+    h->fast = ok;
+  }
   std::vector<c128> tw[3];
   std::vector<int> nat[3];
   for (int ax = 0; ax < 3; ++ax)
@@ -290,7 +332,7 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
 
   lp.ncols = ncols;
   lp.nxl = nxl;
-  lp.colgrp = 16;
+  lp.colgrp = h->fast ? 32 : 16;
   lp.ngrp = (ncols + lp.colgrp - 1) / lp.colgrp;
   lp.ncols_pad = lp.ngrp * lp.colgrp;
   lp.zstride = n3 | 1;
@@ -341,8 +383,58 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     if ((rc = upload(h, plans, &lp.axp, st))) return rc;
   }
 
-  // V_loc / F in digit-permuted positions
-  {
+  int dev = 0, smem_max = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+
+  if (h->fast) {
+    fp.n1 = n1; fp.n2 = n2; fp.n3 = n3;
+    fp.ncols = ncols; fp.ncols_pad = lp.ncols_pad; fp.nxl = nxl;
+    fp.colgrp = lp.colgrp; fp.ngrp = lp.ngrp;
+    fp.zstride = lp.zstride; fp.ystride = lp.ystride;
+    fp.grp_ptr = lp.grp_ptr; fp.ent_pw = lp.ent_pw; fp.ent_off = lp.ent_off; fp.col_hp = lp.col_hp;
+    fp.xl_of_x = lp.xl_of_x; fp.kin = lp.kin;
+    fp.div_colgrp = lp.div_colgrp; fp.div_nxl = lp.div_nxl;
+    // full twiddle tables exp(+2 pi i t / n)
+    const long double PI = 3.14159265358979323846264338327950288L;
+    for (int ax = 0; ax < 3; ++ax) {
+      std::vector<c128> t((size_t)dims[ax]);
+      for (int k = 0; k < dims[ax]; ++k) {
+        const long double ang = 2.0L * PI * (long double)k / (long double)dims[ax];
+        t[k] = cmake((double)cosl(ang), (double)sinl(ang));
+      }
+      if ((rc = upload(h, t, &fp.tw[ax], st))) return rc;
+    }
+    // y-slots per x batch: the largest divisor of n2 that is <= 32 (all of n2 when the x transform is one pass);
+    // shrink it until the plane fits in shared memory; prefer two 256-thread CTAs per SM when they fit
+    if (fp.r2[0] == 1) { fp.yb = n2; fp.tsize = 0; }
+    else {
+      int yb = 1;
+      for (int d = 1; d <= 32 && d <= n2; ++d) if (n2 % d == 0) yb = d;
+      fp.yb = yb; fp.tsize = n1 * yb;
+      while (fast_plane_smem(fp) > (size_t)smem_max && fp.yb > 1) {
+        int nb = 1;
+        for (int d = 1; d < fp.yb; ++d) if (n2 % d == 0) nb = d;
+        fp.yb = nb; fp.tsize = n1 * nb;
+      }
+    }
+    fp.div_yb = make_fastdiv(fp.yb);
+    if (fast_plane_smem(fp) > (size_t)smem_max || fast_zkernel_smem(fp) > (size_t)smem_max) h->fast = false;
+  }
+  if (h->fast) {
+    int smem_sm = 0;
+    CUDA_TRY(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+    fp.plane_threads = (2 * (fast_plane_smem(fp) + 1024) <= (size_t)smem_sm) ? 256 : 512;
+    double* vp = nullptr;
+    CUDA_TRY(cudaMalloc(&vp, F * sizeof(double)));
+    h->allocs.push_back(vp);
+    k_slot_vloc<<<148 * 4, 256, 0, st>>>(n1, n2, n3, fp.r1[0], fp.r2[0], fp.r1[1], fp.r2[1], fp.r1[2], fp.r2[2], vloc,
+                                         1.0 / (double)F, vp);
+    CUDA_TRY(cudaGetLastError());
+    fp.vslot = vp;
+    CUDA_TRY(fast_kernels_init(fp));
+  } else {
+    // generic path: V_loc / F in digit-permuted positions
     const int* dnat[3];
     for (int ax = 0; ax < 3; ++ax)
       if ((rc = upload(h, nat[ax], &dnat[ax], st))) return rc;
@@ -352,6 +444,10 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     k_permute_vloc<<<148 * 4, 256, 0, st>>>(n1, n2, n3, vloc, dnat[0], dnat[1], dnat[2], 1.0 / (double)F, vp);
     CUDA_TRY(cudaGetLastError());
     lp.vperm = vp;
+    if (plane_smem(lp) > (size_t)smem_max || zkernel_smem(lp) > (size_t)smem_max)
+      return fail(PWH_EUNSUPPORTED, "FFT box %dx%dx%d needs %zu bytes of shared memory per plane (limit %d)", n1, n2, n3,
+                  plane_smem(lp), smem_max);
+    CUDA_TRY(local_kernels_init(lp));
   }
 
   // D (copied)
@@ -361,14 +457,6 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     CUDA_TRY(cudaMemcpyAsync(h->dij, dij, nproj * sizeof(double), cudaMemcpyDeviceToDevice, st));
   }
 
-  // shared-memory budgets
-  int dev = 0, smem_max = 0;
-  CUDA_TRY(cudaGetDevice(&dev));
-  CUDA_TRY(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-  if (plane_smem(lp) > (size_t)smem_max || zkernel_smem(lp) > (size_t)smem_max)
-    return fail(PWH_EUNSUPPORTED, "FFT box %dx%dx%d needs %zu bytes of shared memory per plane (limit %d)", n1, n2, n3,
-                plane_smem(lp), smem_max);
-  CUDA_TRY(local_kernels_init(lp));
   CUDA_TRY(zgemm_init());
 
   // bands per launch of the local kernels: keep the column buffer around 48 MB (L2-resident) but at least 2 waves
@@ -450,10 +538,17 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
     launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, y, ldy, h->dij, cmat, h->nproj, ws + w.part, st);
   for (int64_t b0 = 0; b0 < nband; b0 += w.group) {
     const int nb = (int)std::min<int64_t>(w.group, nband - b0);
-    launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, colbuf, nb, st);
-    launch_plane(h->lp, colbuf, nb, st);
-    launch_zfwd_gather(h->lp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
-                       out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+    if (h->fast) {
+      launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, colbuf, nb, st);
+      launch_fast_plane(h->fp, colbuf, nb, st);
+      launch_fast_zfwd_gather(h->fp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                              out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+    } else {
+      launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, colbuf, nb, st);
+      launch_plane(h->lp, colbuf, nb, st);
+      launch_zfwd_gather(h->lp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                         out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+    }
   }
   if (h->nproj > 0)
     launch_zgemm_nn_acc(h->npw, nband, h->nproj, alpha, h->proj, h->ldp, cmat, h->nproj, out, ldout, st);

@@ -89,6 +89,9 @@ RANDOM_CASES = [
     ((6, 6, 6), (4.0, 4.0, 4.0), (0.1, 0.2, 0.3), 1.5, 1, 1),               # 5 plane waves, one band, one projector
     ((64, 40, 36), (14.0, 9.0, 8.0), (0.25, 0.25, 0.25), 6.0, 0, 9),        # no projectors
     ((2, 2, 2), (2.0, 2.0, 2.0), (0.0, 0.0, 0.0), 0.1, 2, 2),               # one plane wave, smallest box
+    ((125, 6, 4), (30.0, 4.0, 3.0), (0.25, 0.0, 0.0), 2.0, 4, 3),           # 125 = 5^3: generic-stage fallback plan
+    ((15, 16, 45), (6.0, 6.5, 14.0), (0.0, 0.25, 0.0), 4.0, 6, 4),          # single-pass 15 and 16, 45 = 9*5
+    ((180, 120, 8), (75.0, 50.0, 4.0), (0.25, 0.25, 0.25), 3.0, 5, 3),      # cfg 5's axis lengths 15*12 and 12*10
 ]
 
 
@@ -107,6 +110,20 @@ def test_random_boxes_apply_filter_gram(gpu, case):
         y = gpu.cheb_filter(ham, psi.clone(), m, w.a, w.b, w.a0).cpu().numpy()
         ref = oracle.cheb_filter(*ham_args(w), w.psi, m, w.a, w.b, w.a0)
         assert relerr(y, ref) <= TOL_F, (case, m)
+    ham.destroy()
+
+
+def test_generic_fft_fallback_cfg2(gpu, cfg2, monkeypatch):
+    """The radix-2/3/4/5/8 shared-memory stage plan (used when an axis does not factor as r1*r2) on config 2."""
+    monkeypatch.setenv("PWH_FORCE_GENERIC_FFT", "1")
+    w = cfg2
+    ham = setup(gpu, w)
+    monkeypatch.delenv("PWH_FORCE_GENERIC_FFT")
+    psi = w.psi[:40]
+    out = gpu.apply_h(ham, to_dev(psi)).cpu().numpy()
+    assert relerr(out, oracle.apply_h(*ham_args(w), psi)) <= TOL_H
+    y = gpu.cheb_filter(ham, to_dev(psi), 3, w.a, w.b, w.a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(w), psi, 3, w.a, w.b, w.a0)) <= TOL_F
     ham.destroy()
 
 

@@ -7,13 +7,22 @@
 // (measured on B200: DMMA.8x8x4 peak 37.1 TFLOP/s == DFMA peak).  One complex product is four real DMMAs on
 // split re/im fragments; operands are staged gmem -> smem with a 4-stage cp.async pipeline in padded layouts
 // that make every 16-byte fragment load conflict-free.
+#include <algorithm>
+#include <cstdlib>
+
 #include "launch.h"
 
 namespace pwh {
 
 namespace {
 
-constexpr int BM = 128, BN = 64, BK = 8, STAGES = 4, NT = 256;
+#ifndef PWH_BK
+#define PWH_BK 8
+#endif
+#ifndef PWH_STAGES
+#define PWH_STAGES 4
+#endif
+constexpr int BM = 128, BN = 64, BK = PWH_BK, STAGES = PWH_STAGES, NT = 256;
 constexpr int WARPS_M = 4, WARPS_N = 2;               // 8 warps, warp tile 32 x 32 complex
 constexpr int KROW = BK * 16 + 64;                     // bytes per row of a K-major tile (== 64 mod 128)
 constexpr int MROW = BM * 16 + 32;                     // bytes per k-row of an M-major A tile (== 32 mod 128)
@@ -178,6 +187,153 @@ k_zgemm(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* _
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// 3M variant: one complex product as THREE real DMMA products instead of four,
+//     T1 = ar.br,  T2 = ai.bi,  T3 = (ar + ai).(br + bi)   =>   re = T1 - T2,  im = T3 - T1 - T2
+// (for conj(a): ai -> -ai).  16 warps (4 x 4), warp tile 32 x 16 complex, three accumulator sets of 16 doubles;
+// the sums ar+ai / br+bi are formed on the fragments (one DADD per fragment element).  Same shared-memory tile
+// layouts and cp.async pipeline as k_zgemm.  The imaginary part carries a rounding error of order
+// eps.(|ar|+|ai|).(|br|+|bi|), i.e. norm-wise the same as the 4M product.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int NT3 = 512;
+constexpr int W3_M = 4, W3_N = 4;                      // warp grid; warp tile 32 x 16
+
+template <bool A_KMAJOR, int EPI>
+__global__ void __launch_bounds__(NT3, 1)
+k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* __restrict__ A, int64_t lda,
+          const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  constexpr int A_BYTES = A_KMAJOR ? A_BYTES_K : A_BYTES_M;
+  constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp % W3_M, wn = warp / W3_M;
+  int tm, tn;
+  if (A_KMAJOR) { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
+  else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
+  const int m0 = tm * BM, n0 = tn * BN;
+  const int split = blockIdx.y;
+  const int64_t kbeg = (int64_t)split * k_per_split;
+  const int64_t kend = (kbeg + k_per_split < K) ? kbeg + k_per_split : K;
+  const int nkt = (int)((kend - kbeg + BK - 1) / BK);
+
+  auto load_stage = [&](int stage, int kt) {
+    const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
+    const int64_t k0 = kbeg + (int64_t)kt * BK;
+    if (A_KMAJOR) {
+#pragma unroll
+      for (int i = 0; i < (BM * BK) / NT3; ++i) {
+        const int idx = tid + i * NT3, r = idx / BK, kk = idx % BK;
+        const bool ok = (m0 + r < M) && (k0 + kk < kend);
+        const c128* src = ok ? A + (int64_t)(m0 + r) * lda + k0 + kk : A;
+        cp_async16(sa + r * KROW + kk * 16, src, ok ? 16 : 0);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < (BM * BK) / NT3; ++i) {
+        const int idx = tid + i * NT3, kk = idx / BM, r = idx % BM;
+        const bool ok = (m0 + r < M) && (k0 + kk < kend);
+        const c128* src = ok ? A + (int64_t)(k0 + kk) * lda + m0 + r : A;
+        cp_async16(sa + kk * MROW + r * 16, src, ok ? 16 : 0);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < (BN * BK) / NT3; ++i) {
+      const int idx = tid + i * NT3, r = idx / BK, kk = idx % BK;
+      const bool ok = (n0 + r < N) && (k0 + kk < kend);
+      const c128* src = ok ? B + (int64_t)(n0 + r) * ldb + k0 + kk : B;
+      cp_async16(sb + r * KROW + kk * 16, src, ok ? 16 : 0);
+    }
+  };
+
+  double t1[4][2][2], t2[4][2][2], t3[4][2][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) { t1[i][j][h] = 0.0; t2[i][j][h] = 0.0; t3[i][j][h] = 0.0; }
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; ++s) {
+    if (s < nkt) load_stage(s, s);
+    cp_async_commit();
+  }
+
+  const int frow = lane >> 2, fk = lane & 3;
+  const uint32_t a_off = A_KMAJOR ? (uint32_t)((wm * 32 + frow) * KROW + fk * 16)
+                                  : (uint32_t)(fk * MROW + (wm * 32 + frow) * 16);
+  const uint32_t b_off = (uint32_t)(A_BYTES + (wn * 16 + frow) * KROW + fk * 16);
+
+  for (int kt = 0; kt < nkt; ++kt) {
+    cp_async_wait<STAGES - 2>();
+#ifndef EXP_NOBAR
+    __syncthreads();
+#endif
+    const uint32_t st = smem_base + (kt % STAGES) * STAGE_BYTES;
+#pragma unroll
+    for (int k4 = 0; k4 < BK / 4; ++k4) {
+      double2 b[2];
+      double sb[2];
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        b[j] = lds128(st + b_off + (uint32_t)(j * 8 * KROW + k4 * 64));
+        sb[j] = b[j].x + b[j].y;
+      }
+      if (k4 == 0) {
+        // refill the stage consumed in the previous iteration (issued after this iteration's first fragment loads
+        // so that the LDGSTS burst does not sit in front of them in the LSU queue)
+        const int nk = kt + STAGES - 1;
+#ifndef EXP_NOLOAD
+        if (nk < nkt) load_stage(nk % STAGES, nk);
+#endif
+        cp_async_commit();
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const uint32_t ao = A_KMAJOR ? (uint32_t)(i * 8 * KROW + k4 * 64) : (uint32_t)(k4 * 4 * MROW + i * 8 * 16);
+        const double2 a = lds128(st + a_off + ao);
+        const double sa = A_KMAJOR ? a.x - a.y : a.x + a.y;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          dmma(t1[i][j][0], t1[i][j][1], a.x, b[j].x);
+          dmma(t2[i][j][0], t2[i][j][1], a.y, b[j].y);
+          dmma(t3[i][j][0], t3[i][j][1], sa, sb[j]);
+        }
+      }
+    }
+  }
+  cp_async_wait<0>();
+
+  c128* Cout = C;
+  if (EPI == EPI_PARTIAL) Cout += (int64_t)split * ldc * N;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int m = m0 + wm * 32 + i * 8 + frow;
+    if (m >= M) continue;
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int n = n0 + wn * 16 + j * 8 + 2 * fk + h;
+        if (n >= N) continue;
+        // conj(a).b : re = T1 + T2, im = T3 - T1 + T2 ;   a.b : re = T1 - T2, im = T3 - T1 - T2
+        const double re = A_KMAJOR ? t1[i][j][h] + t2[i][j][h] : t1[i][j][h] - t2[i][j][h];
+        const double im = A_KMAJOR ? (t3[i][j][h] - t1[i][j][h]) + t2[i][j][h] : (t3[i][j][h] - t1[i][j][h]) - t2[i][j][h];
+        c128* p = Cout + (int64_t)n * ldc + m;
+        if (EPI == EPI_PARTIAL) {
+          *p = cmake(re, im);
+        } else {
+          c128 t = *p;
+          t.x = fma(alpha, re, t.x);
+          t.y = fma(alpha, im, t.y);
+          *p = t;
+        }
+      }
+    }
+  }
+}
+
 // C[m + n*ldc] = scale[m] * sum_s part[s][m + n*M]   (fixed summation order => deterministic)
 __global__ void __launch_bounds__(256) k_splitk_reduce(int M, int N, int nsplit, const c128* __restrict__ part,
                                                        const double* __restrict__ scale, c128* __restrict__ C,
@@ -220,10 +376,20 @@ constexpr int NUM_SMS = 148;
 
 }  // namespace
 
+// PWH_ZGEMM_4M=1 selects the four-product kernels (kept for comparison and as the numerical reference of the 3M ones)
+static bool use_3m() {
+  static const bool v = [] { const char* e = getenv("PWH_ZGEMM_4M"); return !(e && e[0] == '1'); }();
+  return v;
+}
+
 cudaError_t zgemm_init() {
   cudaError_t e = cudaFuncSetAttribute(k_zgemm<true, EPI_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_cn());
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_zgemm<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
+  e = cudaFuncSetAttribute(k_zgemm<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_zgemm3m<true, EPI_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_cn());
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_zgemm3m<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
 }
 
 cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float* ms) {
@@ -245,18 +411,18 @@ cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float
 }
 
 int zgemm_cn_splits(int64_t M, int64_t N, int64_t K) {
+  // Split K so that tiles * splits fills whole waves of the 148 SMs (one CTA per SM): among the candidates with at
+  // most 16 waves and at least 32 k-slabs per split, take the fewest splits within 1 % of the best wave efficiency.
   const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
-  const int64_t max_split = (K + 4 * BK - 1) / (4 * BK);  // at least 4 k-slabs per split
+  const int64_t max_split = std::max<int64_t>(1, K / (32 * BK));
   int best = 1;
   double best_eff = 0.0;
-  for (int waves = 1; waves <= 4; ++waves) {
-    int64_t s = (int64_t)NUM_SMS * waves / tiles;
-    if (s < 1) s = 1;
-    if (s > max_split) s = max_split;
+  for (int64_t s = 1; s <= max_split; ++s) {
     const int64_t ctas = tiles * s;
     const int64_t w = (ctas + NUM_SMS - 1) / NUM_SMS;
+    if (w > 16 && s > 1) break;
     const double eff = (double)ctas / (double)(w * NUM_SMS);
-    if (eff > best_eff + 0.02) { best_eff = eff; best = (int)s; }
+    if (eff > best_eff + 0.01) { best_eff = eff; best = (int)s; }
   }
   return best;
 }
@@ -276,7 +442,10 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
   c128* part = reinterpret_cast<c128*>(ws);
   {
     ScopedLaunch sl(ST_ZGEMM_CN, st);
-    k_zgemm<true, EPI_PARTIAL><<<grid, NT, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
+    if (use_3m())
+      k_zgemm3m<true, EPI_PARTIAL><<<grid, NT3, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
+    else
+      k_zgemm<true, EPI_PARTIAL><<<grid, NT, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
   }
   const int64_t total = M * N;
   int blocks = (int)((total + 255) / 256);
@@ -291,7 +460,10 @@ void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c1
   const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
   dim3 grid(tiles_m * tiles_n, 1);
   ScopedLaunch sl(ST_ZGEMM_NN, st);
-  k_zgemm<false, EPI_ACC><<<grid, NT, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
+  if (use_3m())
+    k_zgemm3m<false, EPI_ACC><<<grid, NT3, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
+  else
+    k_zgemm<false, EPI_ACC><<<grid, NT, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
 }
 
 }  // namespace pwh

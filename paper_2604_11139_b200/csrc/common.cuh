@@ -100,4 +100,18 @@ struct FastPlan {
   FastDiv div_colgrp, div_nxl, div_yb;
 };
 
+// Plan of the size-specialised plane kernel (local_v2.cu).
+struct V2Plan {
+  int n1, n2, n3;
+  int ncols_pad, nxl;
+  int x0;                    // wrapped x of x-line 0: x-line of x is (x - x0) mod n1, touched iff < nxl
+  int variant;               // which template instantiation
+  int r1[2], r2[2], nyb;     // x, y radices and y-slots per warp batch of that instantiation
+  const int2* yrow;          // [n2] per wrapped y: .x = first column - xlmin, .y = xlmin | (count << 16)
+  const c128* twA[2];        // x, y: [r2][r1+1]  exp(+2 pi i s k1 / n) at s (r1+1) + k1
+  const c128* twB[2];        // x, y: [r1][r2+1]  the same value at k1 (r2+1) + s
+  const double* vperm;       // V_loc/F in kernel read order (kv2_perm_vloc)
+  FastDiv div_nxl;
+};
+
 }  // namespace pwh

@@ -38,6 +38,12 @@ void launch_fast_zfwd_gather(const FastPlan& P, const c128* colbuf, const c128* 
                              int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
                              cudaStream_t st);
 
+// local_v2.cu
+bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max);
+cudaError_t v2_kernels_init(const V2Plan& P);
+void launch_v2_perm_vloc(const V2Plan& P, int r1z, int r2z, const double* vloc, double* out, cudaStream_t st);
+void launch_v2_plane(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st);
+
 // zgemm.cu
 cudaError_t zgemm_init();
 // runs `ctas` CTAs x 8 warps x iters x 32 DMMA.8x8x4 (512 flop each) and returns the elapsed milliseconds

@@ -1,0 +1,318 @@
+// local_v2.cu -- size-specialised plane kernel of the local-potential part of H psi.
+//
+//   per (band, z-plane):  disc of touched columns -> inverse y on the touched x-lines -> inverse x -> V_loc(r)/F ->
+//                         forward x (touched x-lines only) -> forward y -> disc
+//
+// Same arithmetic as kf_plane in local_fast.cu (two-pass register-resident transforms, n = r1 * r2, real-space data in
+// "slot" order, V_loc stored once in the order the kernel reads it), re-organised around what the ncu capture of
+// kf_plane showed (profiles/r01b_*): 59 % of its instructions were integer/address work of the generic radix dispatch,
+// its code did not fit the instruction cache, and every pass ended in a CTA-wide barrier with 16 warps resident.
+//   * the box sides and radices are template parameters: every shared-memory access is base + immediate offset;
+//   * the disc is read from and written to global memory directly by the first / last y pass (per-row range tables,
+//     no zero-fill and no staging pass): valid when every y-row of the disc is a contiguous run of x-lines and the
+//     touched x-lines are contiguous modulo n1 (true for any cutoff sphere; checked in pwh_ham_setup, otherwise the
+//     generic kernels are used);
+//   * the x direction is warp-private: a warp owns NYB y-slots at a time and carries them through inverse x,
+//     V_loc multiply and forward x in its own padded buffer with __syncwarp only, so a plane needs 4 CTA barriers;
+//   * V_loc/F is stored as [z-slot][y-batch][q][lane item] so that the multiply reads it fully coalesced.
+#include <type_traits>
+
+#include "fft_reg.cuh"
+#include "launch.h"
+
+namespace pwh {
+
+namespace {
+
+template <int N1_, int R1X_, int R2X_, int N2_, int R1Y_, int R2Y_, int NW_, int NYB_>
+struct PC {
+  static constexpr int N1 = N1_, R1X = R1X_, R2X = R2X_, N2 = N2_, R1Y = R1Y_, R2Y = R2Y_, NW = NW_, NYB = NYB_;
+  static_assert(R1X * R2X == N1 && R1Y * R2Y == N2, "axis factorisation");
+  static_assert(N2 % NYB == 0, "y batches");
+  static constexpr int NT = NW * 32;
+  static constexpr int YS = N2 | 1;                  // odd line stride of the half-plane (elements)
+  static constexpr int XP = R1X * (R2X + 1);         // padded length of one x-line in a warp buffer
+  static constexpr int TWA_X = R2X * (R1X + 1), TWB_X = R1X * (R2X + 1);
+  static constexpr int TWA_Y = R2Y * (R1Y + 1), TWB_Y = R1Y * (R2Y + 1);
+  static constexpr int NBATCH = N2 / NYB;
+  static size_t smem_bytes(int nxl) {
+    return sizeof(c128) * ((size_t)nxl * YS + (size_t)NW * NYB * XP + TWA_X + TWB_X + TWA_Y + TWB_Y) + sizeof(int2) * N2;
+  }
+};
+
+__device__ __forceinline__ c128 czero() { return cmake(0.0, 0.0); }
+
+template <class C>
+__global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __restrict__ colbuf) {
+  constexpr int N1 = C::N1, R1X = C::R1X, R2X = C::R2X, N2 = C::N2, R1Y = C::R1Y, R2Y = C::R2Y;
+  constexpr int NT = C::NT, YS = C::YS, XP = C::XP, NYB = C::NYB;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nxl = P.nxl;
+  c128* half = reinterpret_cast<c128*>(smem_raw);            // [nxl][YS]
+  c128* tbuf = half + nxl * YS;                              // [NW][NYB][XP]
+  c128* twAx = tbuf + C::NW * NYB * XP;                      // [R2X][R1X+1]  w^(s k1)
+  c128* twBx = twAx + C::TWA_X;                              // [R1X][R2X+1]  w^(s k1)
+  c128* twAy = twBx + C::TWB_X;
+  c128* twBy = twAy + C::TWA_Y;
+  int2* yrow = reinterpret_cast<int2*>(twBy + C::TWB_Y);     // [N2]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int zslot = blockIdx.x, band = blockIdx.y;
+
+  for (int i = tid; i < C::TWA_X; i += NT) twAx[i] = P.twA[0][i];
+  for (int i = tid; i < C::TWB_X; i += NT) twBx[i] = P.twB[0][i];
+  for (int i = tid; i < C::TWA_Y; i += NT) twAy[i] = P.twA[1][i];
+  for (int i = tid; i < C::TWB_Y; i += NT) twBy[i] = P.twB[1][i];
+  for (int i = tid; i < N2; i += NT) yrow[i] = P.yrow[i];
+  __syncthreads();
+
+  c128* __restrict__ plane = colbuf + ((int64_t)band * P.n3 + zslot) * P.ncols_pad;
+
+  // ---- y1: inverse y, strided role (radix R1Y over y = q R2Y + s), input straight from the disc in global memory
+  {
+    const int nitems = R2Y * nxl;
+    for (int i = tid; i < nitems; i += NT) {
+      uint32_t s, l;
+      P.div_nxl.divmod((uint32_t)i, s, l);
+      c128 v[R1Y];
+      const int2* yr = yrow + s;
+#pragma unroll
+      for (int q = 0; q < R1Y; ++q) {
+        const int2 row = yr[q * R2Y];
+        const uint32_t d = l - (uint32_t)(row.y & 0xffff);
+        v[q] = d < (uint32_t)(row.y >> 16) ? plane[row.x + (int)l] : czero();
+      }
+      Dft<R1Y, +1>::run(v);
+      const c128* tw = twAy + s * (R1Y + 1);
+      c128* dst = half + l * YS + s;
+      dst[0] = v[0];
+#pragma unroll
+      for (int q = 1; q < R1Y; ++q) dst[q * R2Y] = cmul(v[q], tw[q]);
+    }
+  }
+  __syncthreads();
+  // ---- y2: inverse y, contiguous role (radix R2Y over positions k1 R2Y + s); output in y-slot order
+  {
+    const int nitems = R1Y * nxl;
+    for (int i = tid; i < nitems; i += NT) {
+      uint32_t k1, l;
+      P.div_nxl.divmod((uint32_t)i, k1, l);
+      c128* p = half + l * YS + k1 * R2Y;
+      c128 v[R2Y];
+#pragma unroll
+      for (int q = 0; q < R2Y; ++q) v[q] = p[q];
+      Dft<R2Y, +1>::run(v);
+#pragma unroll
+      for (int q = 0; q < R2Y; ++q) p[q] = v[q];
+    }
+  }
+  __syncthreads();
+
+  // ---- x direction, warp-private: NYB y-slots at a time
+  {
+    c128* tw_ = tbuf + warp * (NYB * XP);
+    const int x0 = P.x0;
+    const double* __restrict__ vz = P.vperm + (int64_t)zslot * ((int64_t)N1 * N2);
+    for (int b = warp; b < C::NBATCH; b += C::NW) {
+      const int y0 = b * NYB;
+      // (a) strided role: radix R1X over x = q R2X + s, twiddle, into the warp buffer at k1 (R2X+1) + s
+      for (int i = lane; i < R2X * NYB; i += 32) {
+        const int s = i % R2X, yb = i / R2X;
+        int xl = s - x0;                       // x-line of x = s (q = 0), modulo N1
+        if (xl < 0) xl += N1;
+        const c128* src = half + y0 + yb;
+        c128 v[R1X];
+#pragma unroll
+        for (int q = 0; q < R1X; ++q) {
+          int xq = xl + q * R2X;
+          if (xq >= N1) xq -= N1;
+          v[q] = xq < nxl ? src[xq * YS] : czero();
+        }
+        Dft<R1X, +1>::run(v);
+        const c128* tw = twAx + s * (R1X + 1);
+        c128* dst = tw_ + yb * XP + s;
+        dst[0] = v[0];
+#pragma unroll
+        for (int q = 1; q < R1X; ++q) dst[q * (R2X + 1)] = cmul(v[q], tw[q]);
+      }
+      __syncwarp();
+      // (b) contiguous role: radix R2X inverse -> real space, multiply by V_loc/F, radix R2X forward, twiddle
+      const double* __restrict__ vb = vz + (int64_t)b * (R2X * R1X * NYB);
+      for (int i = lane; i < R1X * NYB; i += 32) {
+        const int k1 = i % R1X, yb = i / R1X;
+        c128* t = tw_ + yb * XP + k1 * (R2X + 1);
+        c128 v[R2X];
+#pragma unroll
+        for (int q = 0; q < R2X; ++q) v[q] = t[q];
+        Dft<R2X, +1>::run(v);
+#pragma unroll
+        for (int q = 0; q < R2X; ++q) v[q] = cscale(vb[q * (R1X * NYB) + i], v[q]);
+        Dft<R2X, -1>::run(v);
+        const c128* tw = twBx + k1 * (R2X + 1);
+        t[0] = v[0];
+#pragma unroll
+        for (int q = 1; q < R2X; ++q) t[q] = cmulc(v[q], tw[q]);
+      }
+      __syncwarp();
+      // (c) strided role: radix R1X forward over k1, keep the touched x-lines
+      for (int i = lane; i < R2X * NYB; i += 32) {
+        const int s = i % R2X, yb = i / R2X;
+        int xl = s - x0;
+        if (xl < 0) xl += N1;
+        const c128* src = tw_ + yb * XP + s;
+        c128 v[R1X];
+#pragma unroll
+        for (int q = 0; q < R1X; ++q) v[q] = src[q * (R2X + 1)];
+        Dft<R1X, -1>::run(v);
+        c128* dst = half + y0 + yb;
+#pragma unroll
+        for (int q = 0; q < R1X; ++q) {
+          int xq = xl + q * R2X;
+          if (xq >= N1) xq -= N1;
+          if (xq < nxl) dst[xq * YS] = v[q];
+        }
+      }
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+
+  // ---- y2': forward y, contiguous role (radix R2Y over k2 at positions k1 R2Y + k2), twiddle w^-(s k1)
+  {
+    const int nitems = R1Y * nxl;
+    for (int i = tid; i < nitems; i += NT) {
+      uint32_t k1, l;
+      P.div_nxl.divmod((uint32_t)i, k1, l);
+      c128* p = half + l * YS + k1 * R2Y;
+      c128 v[R2Y];
+#pragma unroll
+      for (int q = 0; q < R2Y; ++q) v[q] = p[q];
+      Dft<R2Y, -1>::run(v);
+      const c128* tw = twBy + k1 * (R2Y + 1);
+      p[0] = v[0];
+#pragma unroll
+      for (int q = 1; q < R2Y; ++q) p[q] = cmulc(v[q], tw[q]);
+    }
+  }
+  __syncthreads();
+  // ---- y1': forward y, strided role (radix R1Y over k1 at positions k1 R2Y + s); output y = q R2Y + s to the disc
+  {
+    const int nitems = R2Y * nxl;
+    for (int i = tid; i < nitems; i += NT) {
+      uint32_t s, l;
+      P.div_nxl.divmod((uint32_t)i, s, l);
+      const c128* src = half + l * YS + s;
+      c128 v[R1Y];
+#pragma unroll
+      for (int q = 0; q < R1Y; ++q) v[q] = src[q * R2Y];
+      Dft<R1Y, -1>::run(v);
+      const int2* yr = yrow + s;
+#pragma unroll
+      for (int q = 0; q < R1Y; ++q) {
+        const int2 row = yr[q * R2Y];
+        const uint32_t d = l - (uint32_t)(row.y & 0xffff);
+        if (d < (uint32_t)(row.y >> 16)) plane[row.x + (int)l] = v[q];
+      }
+    }
+  }
+}
+
+// V_loc/F in the order kv2_plane reads it:
+//   out[((zs * NBATCH + b) * R2X + q) * (R1X*NYB) + i],  i = k1 + R1X * yb
+//     = v[x + n1 * (y + n2 * z)] / F   with  x = k1 + R1X q,  y = slot(b NYB + yb; R1Y, R2Y),  z = slot(zs; r1z, r2z),
+//   slot(p; r1, r2) = p / r2 + r1 * (p % r2)
+__global__ void kv2_perm_vloc(int n1, int n2, int n3, int r1x, int r2x, int r1y, int r2y, int r1z, int r2z, int nyb,
+                              const double* __restrict__ v, double inv_f, double* __restrict__ out) {
+  const int64_t total = (int64_t)n1 * n2 * n3;
+  const int per_q = r1x * nyb, per_b = r2x * per_q, nbatch = n2 / nyb;
+  for (int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; o < total; o += (int64_t)gridDim.x * blockDim.x) {
+    const int i = (int)(o % per_q);
+    const int q = (int)((o / per_q) % r2x);
+    const int b = (int)((o / per_b) % nbatch);
+    const int zs = (int)(o / ((int64_t)per_b * nbatch));
+    const int k1 = i % r1x, yb = i / r1x;
+    const int x = k1 + r1x * q;
+    const int p = b * nyb + yb;
+    const int y = p / r2y + r1y * (p % r2y);
+    const int z = zs / r2z + r1z * (zs % r2z);
+    out[o] = v[x + (int64_t)n1 * (y + (int64_t)n2 * z)] * inv_f;
+  }
+}
+
+template <class C>
+cudaError_t v2_init(int nxl) {
+  return cudaFuncSetAttribute(kv2_plane<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes(nxl));
+}
+template <class C>
+void v2_launch(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st) {
+  dim3 grid(P.n3, nb);
+  kv2_plane<C><<<grid, C::NT, C::smem_bytes(P.nxl), st>>>(P, colbuf);
+}
+
+// the specialisations: box side -> (r1, r2) and the (warps, y-slots per warp batch) variants tried in this order
+using C48 = PC<48, 8, 6, 48, 8, 6, 8, 16>;
+using C96a = PC<96, 12, 8, 96, 12, 8, 16, 4>;
+using C96b = PC<96, 12, 8, 96, 12, 8, 8, 4>;
+using C120a = PC<120, 15, 8, 120, 15, 8, 10, 4>;
+using C120b = PC<120, 15, 8, 120, 15, 8, 8, 4>;
+using C128a = PC<128, 16, 8, 128, 16, 8, 16, 4>;
+using C128b = PC<128, 16, 8, 128, 16, 8, 8, 4>;
+
+template <class F>
+bool v2_dispatch(int variant, F&& f) {
+  switch (variant) {
+    case 1: f(C48()); return true;
+    case 2: f(C96a()); return true;
+    case 3: f(C96b()); return true;
+    case 4: f(C120a()); return true;
+    case 5: f(C120b()); return true;
+    case 6: f(C128a()); return true;
+    case 7: f(C128b()); return true;
+    default: return false;
+  }
+}
+
+}  // namespace
+
+// Picks the specialisation for an n1 x n2 plane with nxl touched x-lines that fits `smem_max` bytes of shared memory;
+// fills the radices, NYB and the variant id of the plan.  Returns false when no specialisation applies.
+bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max) {
+  if (n1 != n2) return false;
+  int first = 0, last = -1;
+  if (n1 == 48) { first = last = 1; }
+  else if (n1 == 96) { first = 2; last = 3; }
+  else if (n1 == 120) { first = 4; last = 5; }
+  else if (n1 == 128) { first = 6; last = 7; }
+  for (int var = first; var <= last; ++var) {
+    bool ok = false;
+    v2_dispatch(var, [&](auto c) {
+      using C = decltype(c);
+      if (C::smem_bytes(nxl) <= smem_max) {
+        ok = true;
+        P.variant = var;
+        P.r1[0] = C::R1X; P.r2[0] = C::R2X; P.r1[1] = C::R1Y; P.r2[1] = C::R2Y;
+        P.nyb = C::NYB;
+      }
+    });
+    if (ok) return true;
+  }
+  return false;
+}
+
+cudaError_t v2_kernels_init(const V2Plan& P) {
+  cudaError_t e = cudaErrorInvalidValue;
+  v2_dispatch(P.variant, [&](auto c) { e = v2_init<decltype(c)>(P.nxl); });
+  return e;
+}
+
+void launch_v2_perm_vloc(const V2Plan& P, int r1z, int r2z, const double* vloc, double* out, cudaStream_t st) {
+  const double inv_f = 1.0 / ((double)P.n1 * P.n2 * P.n3);
+  kv2_perm_vloc<<<148 * 4, 256, 0, st>>>(P.n1, P.n2, P.n3, P.r1[0], P.r2[0], P.r1[1], P.r2[1], r1z, r2z, P.nyb, vloc,
+                                         inv_f, out);
+}
+
+void launch_v2_plane(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st) {
+  ScopedLaunch sl(ST_PLANE, st);
+  v2_dispatch(P.variant, [&](auto c) { v2_launch<decltype(c)>(P, colbuf, nb, st); });
+}
+
+}  // namespace pwh

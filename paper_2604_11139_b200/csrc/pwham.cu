@@ -79,6 +79,8 @@ struct pwh_ham {
   LocalPlan lp;
   FastPlan fp;
   bool fast = false;
+  V2Plan vp;
+  bool v2 = false;
   const c128* proj = nullptr;
   int64_t ldp = 0;
   double* dij = nullptr;
@@ -421,6 +423,57 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     fp.div_yb = make_fastdiv(fp.yb);
     if (fast_plane_smem(fp) > (size_t)smem_max || fast_zkernel_smem(fp) > (size_t)smem_max) h->fast = false;
   }
+  // size-specialised plane kernel (local_v2.cu): needs the register-resident z kernels, a box side it is instantiated
+  // for, x-lines contiguous modulo n1 and every y-row of the disc a contiguous run of x-lines
+  if (h->fast) {
+    const char* off = getenv("PWH_NO_V2");
+    V2Plan& vp = h->vp;
+    memset(&vp, 0, sizeof(vp));
+    bool ok = !(off && off[0] == '1') && nxl < 65536 && ncols < (1 << 30);
+    for (int i = 0; i < nxl && ok; ++i) ok = x_of_xl[i] == (x_of_xl[0] + i) % n1;
+    std::vector<int2> yrow((size_t)n2, make_int2(0, 0));
+    if (ok) {
+      std::vector<int> row_gy(n2, INT32_MAX), row_first(n2, 0), row_xlmin(n2, 0), row_cnt(n2, 0);
+      for (int r = 0; r < ncols && ok; ++r) {
+        const Col& c = cols[order[r]];
+        const int xl = xl_of_x[c.xw];
+        if (row_cnt[c.yw] == 0) { row_gy[c.yw] = c.gy; row_first[c.yw] = r; row_xlmin[c.yw] = xl; row_cnt[c.yw] = 1; }
+        else {
+          ok = row_gy[c.yw] == c.gy && r == row_first[c.yw] + row_cnt[c.yw] && xl == row_xlmin[c.yw] + row_cnt[c.yw];
+          row_cnt[c.yw]++;
+        }
+      }
+      for (int y = 0; y < n2; ++y) yrow[y] = make_int2(row_first[y] - row_xlmin[y], row_xlmin[y] | (row_cnt[y] << 16));
+    }
+    if (ok) ok = v2_select(vp, n1, n2, nxl, (size_t)smem_max);
+    if (ok) {
+      vp.n1 = n1; vp.n2 = n2; vp.n3 = n3; vp.ncols_pad = lp.ncols_pad; vp.nxl = nxl; vp.x0 = x_of_xl[0];
+      vp.div_nxl = lp.div_nxl;
+      if ((rc = upload(h, yrow, &vp.yrow, st))) return rc;
+      const long double PI = 3.14159265358979323846264338327950288L;
+      for (int ax = 0; ax < 2; ++ax) {
+        const int n = dims[ax], r1 = vp.r1[ax], r2 = vp.r2[ax];
+        std::vector<c128> ta((size_t)r2 * (r1 + 1), cmake(0.0, 0.0)), tb((size_t)r1 * (r2 + 1), cmake(0.0, 0.0));
+        for (int s = 0; s < r2; ++s)
+          for (int k1 = 0; k1 < r1; ++k1) {
+            const long double ang = 2.0L * PI * (long double)((s * k1) % n) / (long double)n;
+            const c128 w = cmake((double)cosl(ang), (double)sinl(ang));
+            ta[(size_t)s * (r1 + 1) + k1] = w;
+            tb[(size_t)k1 * (r2 + 1) + s] = w;
+          }
+        if ((rc = upload(h, ta, &vp.twA[ax], st))) return rc;
+        if ((rc = upload(h, tb, &vp.twB[ax], st))) return rc;
+      }
+      double* vperm = nullptr;
+      CUDA_TRY(cudaMalloc(&vperm, F * sizeof(double)));
+      h->allocs.push_back(vperm);
+      launch_v2_perm_vloc(vp, fp.r1[2], fp.r2[2], vloc, vperm, st);
+      CUDA_TRY(cudaGetLastError());
+      vp.vperm = vperm;
+      CUDA_TRY(v2_kernels_init(vp));
+      h->v2 = true;
+    }
+  }
   if (h->fast) {
     int smem_sm = 0;
     CUDA_TRY(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
@@ -540,7 +593,8 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
     const int nb = (int)std::min<int64_t>(w.group, nband - b0);
     if (h->fast) {
       launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, colbuf, nb, st);
-      launch_fast_plane(h->fp, colbuf, nb, st);
+      if (h->v2) launch_v2_plane(h->vp, colbuf, nb, st);
+      else launch_fast_plane(h->fp, colbuf, nb, st);
       launch_fast_zfwd_gather(h->fp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
                               out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
     } else {

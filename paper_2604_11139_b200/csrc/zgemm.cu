@@ -38,6 +38,23 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
 }
+// mbarrier helpers (shared-memory barriers that replace the CTA-wide __syncthreads() of the k loop)
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared.b64 st, [%0];\n}\n" ::"r"(bar) : "memory");
+}
+// arrive on `bar` once all cp.async issued so far by this thread have landed (does not change the pending count)
+__device__ __forceinline__ void cp_async_arrive(uint32_t bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(bar), "r"(parity) : "memory");
+}
 __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
       : "+d"(c0), "+d"(c1)
@@ -188,26 +205,44 @@ k_zgemm(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* _
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// 3M variant: one complex product as THREE real DMMA products instead of four,
+// 3M variant (the default): one complex product as THREE real DMMA products instead of four,
 //     T1 = ar.br,  T2 = ai.bi,  T3 = (ar + ai).(br + bi)   =>   re = T1 - T2,  im = T3 - T1 - T2
 // (for conj(a): ai -> -ai).  16 warps (4 x 4), warp tile 32 x 16 complex, three accumulator sets of 16 doubles;
-// the sums ar+ai / br+bi are formed on the fragments (one DADD per fragment element).  Same shared-memory tile
-// layouts and cp.async pipeline as k_zgemm.  The imaginary part carries a rounding error of order
-// eps.(|ar|+|ai|).(|br|+|bi|), i.e. norm-wise the same as the 4M product.
+// the sums ar+ai / br+bi are formed on the fragments (one DADD per fragment element).  The imaginary part carries a
+// rounding error of order eps.(|ar|+|ai|).(|br|+|bi|), i.e. norm-wise the same as the 4M product.
+//
+// There is no CTA-wide barrier in the k loop: stage s is handed over through two shared-memory mbarriers, full[s]
+// (all 512 threads' cp.async of the slab have landed; cp.async.mbarrier.arrive.noinc) and empty[s] (all 16 warps are
+// done reading it), so warps drift by up to one k-slab instead of meeting at every slab (ncu, profiles/r01c: 13 % of
+// the stall samples sat on that __syncthreads; measured CN 38.4 -> 41.3 TFLOP/s, NN 35.4 -> 38.2 at cfg 4).
+// A persistent variant that walks over tiles with the pipeline running across tile boundaries was measured too and
+// was no faster (NN 37.5 vs 38.1), so one CTA computes one tile.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int NT3 = 512;
 constexpr int W3_M = 4, W3_N = 4;                      // warp grid; warp tile 32 x 16
 
-template <bool A_KMAJOR, int EPI>
+template <int BK_>
+struct Tile3 {
+  static constexpr int BK = BK_;
+  static constexpr int KROW = BK * 16 + 64;            // bytes per row of a K-major tile (== 64 mod 128)
+  static constexpr int MROW = BM * 16 + 32;            // bytes per k-row of an M-major A tile (== 32 mod 128)
+  static constexpr int A_K = BM * KROW, A_M = BK * MROW, B_ = BN * KROW;
+};
+
+template <bool A_KMAJOR, int EPI, int BK_, int STAGES_>
 __global__ void __launch_bounds__(NT3, 1)
 k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* __restrict__ A, int64_t lda,
           const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha) {
+  using T = Tile3<BK_>;
+  constexpr int BK = BK_, STAGES = STAGES_, KROW = T::KROW, MROW = T::MROW;
   extern __shared__ __align__(128) unsigned char smem[];
-  constexpr int A_BYTES = A_KMAJOR ? A_BYTES_K : A_BYTES_M;
-  constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  constexpr int A_BYTES = A_KMAJOR ? T::A_K : T::A_M;
+  constexpr int STAGE_BYTES = A_BYTES + T::B_;
   const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp % W3_M, wn = warp / W3_M;
+  // CN: m-tile fastest (all tiles of one K split are co-resident and share the streamed K range through L2)
+  // NN: n-tile fastest (the CTAs that share one slab of A rows run together)
   int tm, tn;
   if (A_KMAJOR) { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
   else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
@@ -254,11 +289,16 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
 #pragma unroll
       for (int h = 0; h < 2; ++h) { t1[i][j][h] = 0.0; t2[i][j][h] = 0.0; t3[i][j][h] = 0.0; }
 
+  // slab kt lives in stage kt % STAGES; its full / empty phase number is kt / STAGES
+  const uint32_t bar_full = smem_base + STAGES * STAGE_BYTES, bar_empty = bar_full + STAGES * 8;
+  if (tid == 0) {
 #pragma unroll
-  for (int s = 0; s < STAGES - 1; ++s) {
-    if (s < nkt) load_stage(s, s);
-    cp_async_commit();
+    for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, NT3); mbar_init(bar_empty + 8 * s, NT3 / 32); }
   }
+  __syncthreads();
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; ++s)
+    if (s < nkt) { load_stage(s, s); cp_async_arrive(bar_full + 8 * s); }
 
   const int frow = lane >> 2, fk = lane & 3;
   const uint32_t a_off = A_KMAJOR ? (uint32_t)((wm * 32 + frow) * KROW + fk * 16)
@@ -266,10 +306,7 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
   const uint32_t b_off = (uint32_t)(A_BYTES + (wn * 16 + frow) * KROW + fk * 16);
 
   for (int kt = 0; kt < nkt; ++kt) {
-    cp_async_wait<STAGES - 2>();
-#ifndef EXP_NOBAR
-    __syncthreads();
-#endif
+    mbar_wait(bar_full + 8 * (kt % STAGES), (uint32_t)(kt / STAGES) & 1u);
     const uint32_t st = smem_base + (kt % STAGES) * STAGE_BYTES;
 #pragma unroll
     for (int k4 = 0; k4 < BK / 4; ++k4) {
@@ -284,10 +321,11 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
         // refill the stage consumed in the previous iteration (issued after this iteration's first fragment loads
         // so that the LDGSTS burst does not sit in front of them in the LSU queue)
         const int nk = kt + STAGES - 1;
-#ifndef EXP_NOLOAD
-        if (nk < nkt) load_stage(nk % STAGES, nk);
-#endif
-        cp_async_commit();
+        if (nk < nkt) {
+          if (kt >= 1) mbar_wait(bar_empty + 8 * (nk % STAGES), (uint32_t)((kt - 1) / STAGES) & 1u);
+          load_stage(nk % STAGES, nk);
+          cp_async_arrive(bar_full + 8 * (nk % STAGES));
+        }
       }
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
@@ -302,6 +340,8 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
         }
       }
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_empty + 8 * (kt % STAGES));
   }
   cp_async_wait<0>();
 
@@ -372,6 +412,11 @@ __global__ void __launch_bounds__(256) k_dmma_probe(int iters, double* __restric
 
 constexpr int smem_cn() { return STAGES * (A_BYTES_K + B_BYTES); }
 constexpr int smem_nn() { return STAGES * (A_BYTES_M + B_BYTES); }
+// 3M kernels: CN streams K = npw in slabs of 8 through 4 stages, NN (K = nproj) in slabs of 16 through 3 stages
+// (measured on B200, cfg 3/4: CN 41.3 vs 40.7 TFLOP/s and NN 35.7 vs 38.2 for slabs of 8 vs 16)
+constexpr int CN3_BK = 8, CN3_STAGES = 4, NN3_BK = 16, NN3_STAGES = 3;
+constexpr int smem_cn3() { return CN3_STAGES * (Tile3<CN3_BK>::A_K + Tile3<CN3_BK>::B_) + 2 * CN3_STAGES * 8; }
+constexpr int smem_nn3() { return NN3_STAGES * (Tile3<NN3_BK>::A_M + Tile3<NN3_BK>::B_) + 2 * NN3_STAGES * 8; }
 constexpr int NUM_SMS = 148;
 
 }  // namespace
@@ -387,9 +432,11 @@ cudaError_t zgemm_init() {
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_zgemm<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_zgemm3m<true, EPI_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_cn());
+  e = cudaFuncSetAttribute(k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           smem_cn3());
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_zgemm3m<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
+  return cudaFuncSetAttribute(k_zgemm3m<false, EPI_ACC, NN3_BK, NN3_STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              smem_nn3());
 }
 
 cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float* ms) {
@@ -443,7 +490,8 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
   {
     ScopedLaunch sl(ST_ZGEMM_CN, st);
     if (use_3m())
-      k_zgemm3m<true, EPI_PARTIAL><<<grid, NT3, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
+      k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES><<<grid, NT3, smem_cn3(), st>>>(
+          (int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
     else
       k_zgemm<true, EPI_PARTIAL><<<grid, NT, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
   }
@@ -461,7 +509,8 @@ void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c1
   dim3 grid(tiles_m * tiles_n, 1);
   ScopedLaunch sl(ST_ZGEMM_NN, st);
   if (use_3m())
-    k_zgemm3m<false, EPI_ACC><<<grid, NT3, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
+    k_zgemm3m<false, EPI_ACC, NN3_BK, NN3_STAGES><<<grid, NT3, smem_nn3(), st>>>(
+        (int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
   else
     k_zgemm<false, EPI_ACC><<<grid, NT, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
 }

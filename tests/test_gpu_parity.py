@@ -300,3 +300,46 @@ def test_host_entry_points(gpu, cfg2):
     assert relerr(hz_h.numpy(), ref_hy) <= TOL_F
     assert relerr(g_h.numpy().T, oracle.gram(ref_y, ref_hy)) <= TOL_F
     ham.destroy()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times
+# ----------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,sample", [(3, (0, 255, 511)), (4, (0, 517, 1023)), (5, (3, 2047))])
+def test_full_size_sampled_bands(gpu, cfg, sample):
+    """Configs 3-5 with ALL their bands, driven exactly as bench.py's step drives them (filter of the config's degree in
+    column blocks of `block`, H.Psi in the same blocks, Gram of the whole block), checked on sampled outputs the oracle
+    can compute one by one: bands never interact before gram, so the oracle filters the
+    sampled bands alone; a Gram entry is one dot product of two such bands.  The samples sit in
+    different band groups of the local kernels, different column blocks and at both ends of the ZGEMM tiles."""
+    import torch
+    w = synth.make_workload(cfg, qr="torch-cuda")
+    spec = w.spec
+    assert w.npw == synth.EXPECTED_NPW[cfg] and w.psi.shape[0] == spec.nband
+    ham = setup(gpu, w)
+    psi = to_dev(w.psi)
+    hpsi = torch.empty_like(psi)
+    for b0 in range(0, spec.nband, spec.block):
+        gpu.cheb_filter(ham, psi[b0:b0 + spec.block], spec.degree, w.a, w.b, w.a0)
+    for b0 in range(0, spec.nband, spec.block):
+        gpu.apply_h(ham, psi[b0:b0 + spec.block], hpsi[b0:b0 + spec.block])
+    g = gpu.gram(psi, hpsi)
+    torch.cuda.synchronize()
+    idx = list(sample)
+    y_gpu = psi[idx].cpu().numpy()
+    hy_gpu = hpsi[idx].cpu().numpy()
+    g_gpu = g[idx][:, idx].cpu().numpy()
+    g_scale = float(g.abs().max())
+    ham.destroy()
+    del psi, hpsi, g
+
+    y_ref = oracle.cheb_filter(*ham_args(w), w.psi[idx], spec.degree, w.a, w.b, w.a0)
+    hy_ref = oracle.apply_h(*ham_args(w), y_ref)
+    g_ref = oracle.gram(y_ref, hy_ref)
+    for k in range(len(idx)):                     # band by band, each against its own norm
+        assert relerr(y_gpu[k], y_ref[k]) <= TOL_F
+        assert relerr(hy_gpu[k], hy_ref[k]) <= TOL_F      # H applied to the filtered band inherits the filter's error
+    # H alone at TOL_H: the GPU's H applied to the GPU's filtered bands against the oracle's H applied to the same input
+    assert relerr(hy_gpu, oracle.apply_h(*ham_args(w), y_gpu)) <= TOL_H
+    assert relerr(g_gpu, oracle.gram(y_gpu, hy_gpu)) <= TOL_H
+    assert np.abs(g_gpu - g_ref).max() <= TOL_F * g_scale

@@ -114,4 +114,17 @@ struct V2Plan {
   FastDiv div_nxl;
 };
 
+// Plan of the warp-private z kernels (local_z.cu): n3 = r1 * r2, a work item is (cw columns, one band).
+struct ZPlan {
+  int n3, r1, r2;
+  int r1p;                   // r1 rounded up to a multiple of 4 (row length of ztab)
+  int cw, log2cw;            // columns per work item (power of two: 4 when r2 >= 6), its log2
+  int nq;                    // work items per band = ncols_pad / cw
+  int ncols_pad;
+  int zs;                    // elements per column of a warp buffer; position of z = q r2 + s is q (r2 + 1) + s
+  const int* ztab;           // [nq][r2][cw][r1p]: plane-wave index of column quad*cw + c at z = q r2 + sub, -1 outside
+  const c128* tw;            // tw[t] = exp(+2 pi i t / n3)
+  const double* kin;         // [npw]
+};
+
 }  // namespace pwh

@@ -44,6 +44,14 @@ cudaError_t v2_kernels_init(const V2Plan& P);
 void launch_v2_perm_vloc(const V2Plan& P, int r1z, int r2z, const double* vloc, double* out, cudaStream_t st);
 void launch_v2_plane(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st);
 
+// local_z.cu
+size_t zw_smem(const ZPlan& P);
+cudaError_t zw_kernels_init(const ZPlan& P);
+void launch_zw_scatter_zinv(const ZPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st);
+void launch_zw_zfwd_gather(const ZPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,
+                           int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
+                           cudaStream_t st);
+
 // zgemm.cu
 cudaError_t zgemm_init();
 // runs `ctas` CTAs x 8 warps x iters x 32 DMMA.8x8x4 (512 flop each) and returns the elapsed milliseconds

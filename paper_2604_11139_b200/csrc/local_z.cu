@@ -1,0 +1,238 @@
+// local_z.cu -- warp-private z transforms of the local-potential part of H psi.
+//
+//   kz_scatter_zinv : sphere -> touched z-columns, inverse z transform, store plane-major [band][z-slot][column]
+//
+//   kz_zfwd_gather  : forward z transform of the columns, gather the sphere, fused kinetic + three-term recurrence
+//                     out = alpha * ((kin - c) . y + w_loc) - beta * y_prev
+//
+// Same arithmetic as kf_scatter_zinv / kf_zfwd_gather in local_fast.cu (two-pass register-resident transforms,
+// n3 = r1 * r2), re-organised around what the ncu capture of those kernels showed (profiles/r01c: 21 % of the warp
+// slots, 5-11 long-scoreboard stalls per issue, every phase -- zero-fill, index loads, gather, two passes -- ended by a
+// CTA-wide barrier with all warps in the same phase):
+//   * a work item is (cw columns, one band), owned by ONE warp; its two passes meet in a warp-private shared-memory
+//     buffer with __syncwarp only, so the 16 warps of an SM drift apart and one warp's global-load latency is covered
+//     by the others' butterflies.  Warps walk over the items of the whole band group (persistent grid);
+//   * there is no zero-fill, no staging of the sphere and no index indirection through shared memory: the first pass
+//     of the inverse transform takes its radix-r1 inputs straight from psi through a table of plane-wave indices laid
+//     out in the order the lanes read it (-1 = outside the sphere: the input is zero and is not loaded), and the last
+//     pass of the forward transform holds the r1 outputs of a column in registers and applies the recurrence epilogue
+//     to those that are inside the sphere.  Every global load of a pass is independent of the others (up to 16 + 16
+//     in flight per thread).
+#include <type_traits>
+
+#include "fft_reg.cuh"
+#include "launch.h"
+
+namespace pwh {
+
+namespace {
+
+constexpr int ZW = 8;   // warps per CTA; two CTAs per SM
+
+template <int R>
+using RC = std::integral_constant<int, R>;
+
+template <bool BIG, class F>
+__device__ __forceinline__ void with_radix(int r, F&& f) {
+  switch (r) {
+    case 1: f(RC<1>()); break;
+    case 2: f(RC<2>()); break;
+    case 3: f(RC<3>()); break;
+    case 4: f(RC<4>()); break;
+    case 5: f(RC<5>()); break;
+    case 6: f(RC<6>()); break;
+    case 8: f(RC<8>()); break;
+    case 9: f(RC<9>()); break;
+    case 10: f(RC<10>()); break;
+    case 12: f(RC<12>()); break;
+    case 15: if constexpr (BIG) f(RC<15>()); break;
+    case 16: if constexpr (BIG) f(RC<16>()); break;
+    default: break;
+  }
+}
+
+// table row of one (sub, column): R plane-wave indices padded to a multiple of 4, read as int4
+template <int R>
+__device__ __forceinline__ void load_idx(const int* __restrict__ row, int* idx) {
+  constexpr int R4 = (R + 3) / 4;
+  const int4* r4 = reinterpret_cast<const int4*>(row);
+#pragma unroll
+  for (int i = 0; i < R4; ++i) {
+    const int4 t = __ldg(r4 + i);
+    if (4 * i + 0 < R) idx[4 * i + 0] = t.x;
+    if (4 * i + 1 < R) idx[4 * i + 1] = t.y;
+    if (4 * i + 2 < R) idx[4 * i + 2] = t.z;
+    if (4 * i + 3 < R) idx[4 * i + 3] = t.w;
+  }
+}
+
+__global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, const c128* __restrict__ psi, int64_t ldpsi,
+                                                              c128* __restrict__ colbuf, int nb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  c128* tw = reinterpret_cast<c128*>(smem_raw);                       // [n3]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  c128* buf = tw + P.n3 + warp * (P.cw * P.zs);                       // [cw][zs], warp-private
+  for (int i = tid; i < P.n3; i += ZW * 32) tw[i] = P.tw[i];
+  __syncthreads();
+  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, r1p = P.r1p;
+  const int64_t pstride = P.ncols_pad;
+  const int nitems = P.nq * nb;
+  for (int item = blockIdx.x * ZW + warp; item < nitems; item += gridDim.x * ZW) {
+    const int quad = item % P.nq, band = item / P.nq;
+    const c128* __restrict__ src = psi + (int64_t)band * ldpsi;
+    c128* __restrict__ dst = colbuf + (int64_t)band * P.n3 * pstride + quad * cw;
+    const int* __restrict__ tab = P.ztab + (int64_t)quad * (r2 * cw * r1p);
+    // pass 1, strided role: radix r1 over z = q r2 + sub, inputs gathered from the sphere
+    with_radix<true>(r1, [&](auto rc) {
+      constexpr int R = decltype(rc)::value;
+      for (int i = lane; i < r2 * cw; i += 32) {
+        const int sub = i >> lcw, c = i & (cw - 1);
+        int idx[R];
+        load_idx<R>(tab + (int64_t)i * r1p, idx);
+        c128 v[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = idx[q] >= 0 ? src[idx[q]] : cmake(0.0, 0.0);
+        Dft<R, +1>::run(v);
+        if (r2 == 1) {
+#pragma unroll
+          for (int q = 0; q < R; ++q) dst[(int64_t)q * pstride + c] = v[q];
+        } else {
+          c128* b = buf + c * zs + sub;
+          b[0] = v[0];
+#pragma unroll
+          for (int q = 1; q < R; ++q) b[q * (r2 + 1)] = cmul(v[q], tw[sub * q]);
+        }
+      }
+    });
+    if (r2 == 1) continue;
+    __syncwarp();
+    // pass 2, contiguous role: radix r2 over positions sub r2 + q; output z-slot sub r2 + q, plane-major
+    with_radix<false>(r2, [&](auto rc) {
+      constexpr int R = decltype(rc)::value;
+      for (int i = lane; i < r1 * cw; i += 32) {
+        const int sub = i >> lcw, c = i & (cw - 1);
+        const c128* b = buf + c * zs + sub * (R + 1);
+        c128 v[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = b[q];
+        Dft<R, +1>::run(v);
+        c128* d = dst + (int64_t)(sub * R) * pstride + c;
+#pragma unroll
+        for (int q = 0; q < R; ++q) d[(int64_t)q * pstride] = v[q];
+      }
+    });
+    __syncwarp();
+  }
+}
+
+__global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, const c128* __restrict__ colbuf,
+                                                             const c128* __restrict__ y, int64_t ldy,
+                                                             const c128* __restrict__ yprev, int64_t ldprev,
+                                                             c128* __restrict__ out, int64_t ldout, double alpha,
+                                                             double cshift, double beta, int nb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  c128* tw = reinterpret_cast<c128*>(smem_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  c128* buf = tw + P.n3 + warp * (P.cw * P.zs);
+  for (int i = tid; i < P.n3; i += ZW * 32) tw[i] = P.tw[i];
+  __syncthreads();
+  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, r1p = P.r1p;
+  const int64_t pstride = P.ncols_pad;
+  const double* __restrict__ kin = P.kin;
+  const int nitems = P.nq * nb;
+  for (int item = blockIdx.x * ZW + warp; item < nitems; item += gridDim.x * ZW) {
+    const int quad = item % P.nq, band = item / P.nq;
+    const c128* __restrict__ src = colbuf + (int64_t)band * P.n3 * pstride + quad * cw;
+    const int* __restrict__ tab = P.ztab + (int64_t)quad * (r2 * cw * r1p);
+    const c128* __restrict__ yb = y + (int64_t)band * ldy;
+    const c128* __restrict__ pb = (beta != 0.0) ? yprev + (int64_t)band * ldprev : nullptr;
+    c128* __restrict__ ob = out + (int64_t)band * ldout;
+    if (r2 > 1) {
+      // pass 1, contiguous role: radix r2 over z-slots sub r2 + q, twiddle w^-(sub q)
+      with_radix<false>(r2, [&](auto rc) {
+        constexpr int R = decltype(rc)::value;
+        for (int i = lane; i < r1 * cw; i += 32) {
+          const int sub = i >> lcw, c = i & (cw - 1);
+          const c128* s = src + (int64_t)(sub * R) * pstride + c;
+          c128 v[R];
+#pragma unroll
+          for (int q = 0; q < R; ++q) v[q] = s[(int64_t)q * pstride];
+          Dft<R, -1>::run(v);
+          c128* b = buf + c * zs + sub * (R + 1);
+          b[0] = v[0];
+#pragma unroll
+          for (int q = 1; q < R; ++q) b[q] = cmulc(v[q], tw[sub * q]);
+        }
+      });
+      __syncwarp();
+    }
+    // pass 2, strided role: radix r1 over positions q r2 + sub; output = w_loc at z = q r2 + sub; recurrence epilogue
+    with_radix<true>(r1, [&](auto rc) {
+      constexpr int R = decltype(rc)::value;
+      for (int i = lane; i < r2 * cw; i += 32) {
+        const int sub = i >> lcw, c = i & (cw - 1);
+        int idx[R];
+        load_idx<R>(tab + (int64_t)i * r1p, idx);
+        c128 v[R];
+        if (r2 == 1) {
+#pragma unroll
+          for (int q = 0; q < R; ++q) v[q] = src[(int64_t)q * pstride + c];
+        } else {
+          const c128* b = buf + c * zs + sub;
+#pragma unroll
+          for (int q = 0; q < R; ++q) v[q] = b[q * (r2 + 1)];
+        }
+        Dft<R, -1>::run(v);
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+          const int g = idx[q];
+          if (g < 0) continue;
+          const c128 yv = yb[g];
+          const double k = kin[g] - cshift;
+          c128 r = cmake(alpha * fma(k, yv.x, v[q].x), alpha * fma(k, yv.y, v[q].y));
+          if (pb) {
+            const c128 pv = pb[g];
+            r.x = fma(-beta, pv.x, r.x);
+            r.y = fma(-beta, pv.y, r.y);
+          }
+          ob[g] = r;
+        }
+      }
+    });
+    __syncwarp();
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------------
+size_t zw_smem(const ZPlan& P) { return sizeof(c128) * ((size_t)P.n3 + (size_t)ZW * P.cw * P.zs); }
+
+cudaError_t zw_kernels_init(const ZPlan& P) {
+  cudaError_t e = cudaFuncSetAttribute(kz_scatter_zinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zw_smem(P));
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(kz_zfwd_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zw_smem(P));
+}
+
+static int zw_grid(const ZPlan& P, int nb) {
+  const int64_t items = (int64_t)P.nq * nb;
+  const int64_t ctas = (items + ZW - 1) / ZW;
+  return (int)(ctas < 2 * 148 ? ctas : 2 * 148);     // persistent: two CTAs of 8 warps per SM
+}
+
+void launch_zw_scatter_zinv(const ZPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st) {
+  ScopedLaunch sl(ST_SCATTER_ZINV, st);
+  kz_scatter_zinv<<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, psi, ldpsi, colbuf, nb);
+}
+
+void launch_zw_zfwd_gather(const ZPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,
+                           int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
+                           cudaStream_t st) {
+  ScopedLaunch sl(ST_ZFWD_GATHER, st);
+  kz_zfwd_gather<<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha, cshift,
+                                                             yprev ? beta : 0.0, nb);
+}
+
+}  // namespace pwh

@@ -81,6 +81,8 @@ struct pwh_ham {
   bool fast = false;
   V2Plan vp;
   bool v2 = false;
+  ZPlan zp;
+  bool zw = false;
   const c128* proj = nullptr;
   int64_t ldp = 0;
   double* dij = nullptr;
@@ -474,6 +476,37 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
       h->v2 = true;
     }
   }
+  // warp-private z kernels (local_z.cu): table of plane-wave indices in the order their lanes read it
+  if (h->fast) {
+    const char* off = getenv("PWH_NO_ZW");
+    ZPlan& zp = h->zp;
+    memset(&zp, 0, sizeof(zp));
+    zp.n3 = n3; zp.r1 = fp.r1[2]; zp.r2 = fp.r2[2];
+    zp.r1p = (zp.r1 + 3) / 4 * 4;
+    zp.cw = zp.r2 >= 6 ? 4 : (zp.r2 >= 4 ? 8 : (zp.r2 >= 2 ? 16 : 32));
+    zp.log2cw = zp.cw == 4 ? 2 : (zp.cw == 8 ? 3 : (zp.cw == 16 ? 4 : 5));
+    zp.nq = lp.ncols_pad / zp.cw;
+    zp.ncols_pad = lp.ncols_pad;
+    // column stride of a warp buffer: cw = 4 lanes x 2 consecutive subs of a quarter-warp need stride == 2 (mod 8),
+    // cw >= 8 lanes of a quarter-warp sit on 8 columns and need an odd stride
+    int zs = zp.r1 * (zp.r2 + 1);
+    if (zp.cw == 4) { while (zs % 8 != 2) ++zs; } else zs |= 1;
+    zp.zs = zs;
+    zp.tw = fp.tw[2];
+    zp.kin = lp.kin;
+    if (!(off && off[0] == '1') && zw_smem(zp) <= (size_t)smem_max) {
+      std::vector<int> ztab((size_t)zp.nq * zp.r2 * zp.cw * zp.r1p, -1);
+      for (int64_t i = 0; i < npw; ++i) {
+        const int xw = wrapi(g[3 * i], n1), yw = wrapi(g[3 * i + 1], n2), zw_ = wrapi(g[3 * i + 2], n3);
+        const int c = rank[col_of_xy[(size_t)yw * n1 + xw]];
+        const int quad = c / zp.cw, cl = c % zp.cw, sub = zw_ % zp.r2, q = zw_ / zp.r2;
+        ztab[(((size_t)quad * zp.r2 + sub) * zp.cw + cl) * zp.r1p + q] = (int)i;
+      }
+      if ((rc = upload(h, ztab, &zp.ztab, st))) return rc;
+      CUDA_TRY(zw_kernels_init(zp));
+      h->zw = true;
+    }
+  }
   if (h->fast) {
     int smem_sm = 0;
     CUDA_TRY(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
@@ -592,11 +625,16 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
   for (int64_t b0 = 0; b0 < nband; b0 += w.group) {
     const int nb = (int)std::min<int64_t>(w.group, nband - b0);
     if (h->fast) {
-      launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, colbuf, nb, st);
+      if (h->zw) launch_zw_scatter_zinv(h->zp, y + b0 * ldy, ldy, colbuf, nb, st);
+      else launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, colbuf, nb, st);
       if (h->v2) launch_v2_plane(h->vp, colbuf, nb, st);
       else launch_fast_plane(h->fp, colbuf, nb, st);
-      launch_fast_zfwd_gather(h->fp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+      if (h->zw)
+        launch_zw_zfwd_gather(h->zp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
                               out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+      else
+        launch_fast_zfwd_gather(h->fp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                                out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
     } else {
       launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, colbuf, nb, st);
       launch_plane(h->lp, colbuf, nb, st);

@@ -122,7 +122,8 @@ struct ZPlan {
   int nq;                    // work items per band = ncols_pad / cw
   int ncols_pad;
   int zs;                    // elements per column of a warp buffer; position of z = q r2 + s is q (r2 + 1) + s
-  const int* ztab;           // [nq][r2][cw][r1p]: plane-wave index of column quad*cw + c at z = q r2 + sub, -1 outside
+  const int* ztab;           // [nq][r1p/4][r2*cw][4]: plane-wave index of column quad*cw + c at z = q r2 + sub (element
+                             // sub*cw + c, q = 4 j + k), -1 outside the sphere
   const c128* tw;            // tw[t] = exp(+2 pi i t / n3)
   const double* kin;         // [npw]
 };

@@ -51,18 +51,19 @@ __device__ __forceinline__ void with_radix(int r, F&& f) {
   }
 }
 
-// table row of one (sub, column): R plane-wave indices padded to a multiple of 4, read as int4
+// the R plane-wave indices of work-item element i = sub*cw + c (R padded to a multiple of 4): int4 number j of element i
+// sits at tab4[j * nelem + i], so one load instruction of a warp reads 512 contiguous bytes
 template <int R>
-__device__ __forceinline__ void load_idx(const int* __restrict__ row, int* idx) {
+__device__ __forceinline__ void load_idx(const int4* __restrict__ tab4, int nelem, int i, int* idx) {
   constexpr int R4 = (R + 3) / 4;
-  const int4* r4 = reinterpret_cast<const int4*>(row);
+  const int4* r4 = tab4 + i;
 #pragma unroll
-  for (int i = 0; i < R4; ++i) {
-    const int4 t = __ldg(r4 + i);
-    if (4 * i + 0 < R) idx[4 * i + 0] = t.x;
-    if (4 * i + 1 < R) idx[4 * i + 1] = t.y;
-    if (4 * i + 2 < R) idx[4 * i + 2] = t.z;
-    if (4 * i + 3 < R) idx[4 * i + 3] = t.w;
+  for (int j = 0; j < R4; ++j) {
+    const int4 t = __ldg(r4 + (int64_t)j * nelem);
+    if (4 * j + 0 < R) idx[4 * j + 0] = t.x;
+    if (4 * j + 1 < R) idx[4 * j + 1] = t.y;
+    if (4 * j + 2 < R) idx[4 * j + 2] = t.z;
+    if (4 * j + 3 < R) idx[4 * j + 3] = t.w;
   }
 }
 
@@ -81,14 +82,14 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
     const int quad = item % P.nq, band = item / P.nq;
     const c128* __restrict__ src = psi + (int64_t)band * ldpsi;
     c128* __restrict__ dst = colbuf + (int64_t)band * P.n3 * pstride + quad * cw;
-    const int* __restrict__ tab = P.ztab + (int64_t)quad * (r2 * cw * r1p);
+    const int4* __restrict__ tab4 = reinterpret_cast<const int4*>(P.ztab + (int64_t)quad * (r2 * cw * r1p));
     // pass 1, strided role: radix r1 over z = q r2 + sub, inputs gathered from the sphere
     with_radix<true>(r1, [&](auto rc) {
       constexpr int R = decltype(rc)::value;
       for (int i = lane; i < r2 * cw; i += 32) {
         const int sub = i >> lcw, c = i & (cw - 1);
         int idx[R];
-        load_idx<R>(tab + (int64_t)i * r1p, idx);
+        load_idx<R>(tab4, r2 * cw, i, idx);
         c128 v[R];
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = idx[q] >= 0 ? src[idx[q]] : cmake(0.0, 0.0);
@@ -143,10 +144,21 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
   for (int item = blockIdx.x * ZW + warp; item < nitems; item += gridDim.x * ZW) {
     const int quad = item % P.nq, band = item / P.nq;
     const c128* __restrict__ src = colbuf + (int64_t)band * P.n3 * pstride + quad * cw;
-    const int* __restrict__ tab = P.ztab + (int64_t)quad * (r2 * cw * r1p);
+    const int4* __restrict__ tab4 = reinterpret_cast<const int4*>(P.ztab + (int64_t)quad * (r2 * cw * r1p));
     const c128* __restrict__ yb = y + (int64_t)band * ldy;
     const c128* __restrict__ pb = (beta != 0.0) ? yprev + (int64_t)band * ldprev : nullptr;
     c128* __restrict__ ob = out + (int64_t)band * ldout;
+    // the epilogue's operands y[g], y_prev[g] come from HBM: start them towards L2 now, the transforms run meanwhile
+    for (int i = lane; i < r2 * cw * (r1p / 4); i += 32) {
+      const int4 t = __ldg(tab4 + i);
+      const int gi[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (gi[k] >= 0) {
+          asm volatile("prefetch.global.L2 [%0];\n" ::"l"(yb + gi[k]));
+          if (pb) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(pb + gi[k]));
+        }
+    }
     if (r2 > 1) {
       // pass 1, contiguous role: radix r2 over z-slots sub r2 + q, twiddle w^-(sub q)
       with_radix<false>(r2, [&](auto rc) {
@@ -172,7 +184,7 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
       for (int i = lane; i < r2 * cw; i += 32) {
         const int sub = i >> lcw, c = i & (cw - 1);
         int idx[R];
-        load_idx<R>(tab + (int64_t)i * r1p, idx);
+        load_idx<R>(tab4, r2 * cw, i, idx);
         c128 v[R];
         if (r2 == 1) {
 #pragma unroll

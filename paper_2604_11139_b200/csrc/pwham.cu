@@ -500,7 +500,8 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
         const int xw = wrapi(g[3 * i], n1), yw = wrapi(g[3 * i + 1], n2), zw_ = wrapi(g[3 * i + 2], n3);
         const int c = rank[col_of_xy[(size_t)yw * n1 + xw]];
         const int quad = c / zp.cw, cl = c % zp.cw, sub = zw_ % zp.r2, q = zw_ / zp.r2;
-        ztab[(((size_t)quad * zp.r2 + sub) * zp.cw + cl) * zp.r1p + q] = (int)i;
+        const size_t nelem = (size_t)zp.r2 * zp.cw, el = (size_t)sub * zp.cw + cl;
+        ztab[(((size_t)quad * (zp.r1p / 4) + q / 4) * nelem + el) * 4 + q % 4] = (int)i;
       }
       if ((rc = upload(h, ztab, &zp.ztab, st))) return rc;
       CUDA_TRY(zw_kernels_init(zp));
@@ -545,12 +546,23 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
 
   CUDA_TRY(zgemm_init());
 
-  // bands per launch of the local kernels: keep the column buffer around 48 MB (L2-resident) but at least 2 waves
+  // bands per launch of the local kernels: the column buffer of a group (written by one kernel, read by the next) should
+  // stay in the 126 MB L2 -- at most 56 MB -- and the plane kernel's grid of n3 x bands CTAs (one per SM) should fill
+  // whole waves of the 148 SMs: among the group sizes whose buffer is between 24 and 56 MB take the one with the best
+  // wave efficiency (ncu, profiles/r01d: 7 bands x 128 planes = 6.05 waves left the seventh wave almost empty)
   const size_t per_band = (size_t)n3 * lp.ncols_pad * sizeof(c128);
-  int64_t grp = (int64_t)((48u << 20) / std::max<size_t>(per_band, 1));
   const int64_t min_grp = (2 * 148 + n3 - 1) / n3;
-  grp = std::max<int64_t>(grp, min_grp);
-  grp = std::min<int64_t>(std::max<int64_t>(grp, 1), 4096);
+  int64_t g_lo = std::max<int64_t>(std::max<int64_t>((int64_t)((24u << 20) / std::max<size_t>(per_band, 1)), min_grp), 1);
+  int64_t g_hi = std::max<int64_t>((int64_t)((56u << 20) / std::max<size_t>(per_band, 1)), g_lo);
+  g_hi = std::min<int64_t>(g_hi, 4096);
+  g_lo = std::min<int64_t>(g_lo, g_hi);
+  int64_t grp = g_hi;
+  double best_eff = -1.0;
+  for (int64_t c = g_lo; c <= g_hi; ++c) {
+    const int64_t ctas = c * n3, waves = (ctas + 147) / 148;
+    const double eff = (double)ctas / (double)(waves * 148);
+    if (eff >= best_eff + 0.005 || (eff >= best_eff - 0.005 && c > grp && eff >= 0.97)) { best_eff = std::max(eff, best_eff); grp = c; }
+  }
   h->band_group = (int)grp;
 
   CUDA_TRY(cudaStreamSynchronize(st));

@@ -127,6 +127,24 @@ def test_generic_fft_fallback_cfg2(gpu, cfg2, monkeypatch):
     ham.destroy()
 
 
+@pytest.mark.parametrize("env", [("PWH_NO_ZW",), ("PWH_NO_V2",), ("PWH_NO_ZW", "PWH_NO_V2")])
+def test_fallback_kernels_cfg2(gpu, cfg2, monkeypatch, env):
+    """The CTA-per-column-group z kernels and the generic-size plane kernel (local_fast.cu), which serve boxes the
+    size-specialised kernels are not instantiated for, on config 2."""
+    for e in env:
+        monkeypatch.setenv(e, "1")
+    w = cfg2
+    ham = setup(gpu, w)
+    for e in env:
+        monkeypatch.delenv(e)
+    psi = w.psi[:40]
+    out = gpu.apply_h(ham, to_dev(psi)).cpu().numpy()
+    assert relerr(out, oracle.apply_h(*ham_args(w), psi)) <= TOL_H
+    y = gpu.cheb_filter(ham, to_dev(psi), 3, w.a, w.b, w.a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(w), psi, 3, w.a, w.b, w.a0)) <= TOL_F
+    ham.destroy()
+
+
 def test_cfg3_band_subset(gpu):
     """Config 3 (k = 1/4 1/4 1/4, 96^3, 57925 plane waves, 512 projectors) at full N and J on a subset of bands --
     exact, since bands never interact before gram."""

@@ -7,6 +7,8 @@
 // (measured on B200: DMMA.8x8x4 peak 37.1 TFLOP/s == DFMA peak).  One complex product is four real DMMAs on
 // split re/im fragments; operands are staged gmem -> smem with a 4-stage cp.async pipeline in padded layouts
 // that make every 16-byte fragment load conflict-free.
+#include <cuda.h>
+
 #include <algorithm>
 #include <cstdlib>
 
@@ -73,7 +75,7 @@ template <bool A_KMAJOR, int EPI>
 __global__ void __launch_bounds__(NT, 1)
 k_zgemm(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* __restrict__ A, int64_t lda,
         const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha) {
-  extern __shared__ __align__(128) unsigned char smem[];
+  extern __shared__ __align__(1024) unsigned char smem[];
   constexpr int A_BYTES = A_KMAJOR ? A_BYTES_K : A_BYTES_M;
   constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
   const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
@@ -235,7 +237,7 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
           const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha) {
   using T = Tile3<BK_>;
   constexpr int BK = BK_, STAGES = STAGES_, KROW = T::KROW, MROW = T::MROW;
-  extern __shared__ __align__(128) unsigned char smem[];
+  extern __shared__ __align__(1024) unsigned char smem[];
   constexpr int A_BYTES = A_KMAJOR ? T::A_K : T::A_M;
   constexpr int STAGE_BYTES = A_BYTES + T::B_;
   const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
@@ -374,6 +376,166 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// TMA-fed 3M kernel (the default when the driver exports cuTensorMapEncodeTiled): same warp tiling, 3M arithmetic,
+// mbarrier hand-over and epilogue as k_zgemm3m, but the operand slabs are brought in by the TMA engine
+// (cp.async.bulk.tensor, 128-byte swizzle) instead of 512 threads x 3-6 LDGSTS with their address arithmetic:
+// the instruction stream of the 16 warps is then only wait / LDS / DADD / DMMA, which is what the register-level
+// probe of this loop shows to run at 92 % of the DMMA peak.
+//   * matrices are described to the TMA as FP64 tensors with the (re, im) pair innermost: 8 complex = 128 bytes;
+//   * K-major operands (A of CN, B): box = 8 k x rows, dense rows of 128 B in shared memory, chunk c of row r stored
+//     at chunk c ^ (r & 7); the fragment of k-slot fk at step k4 is physical k = 2 fk + (k4 & 1), which makes the 2 rows
+//     x 4 k of a quarter-warp hit 8 different chunks (any assignment of k to the 4 slots of m8n8k4 is valid as long
+//     as A and B agree);
+//   * M-major A of NN: one box of 8 m x BK k per group of 8 rows, stored [m group][k][8 m], chunk m stored at
+//     m ^ (k & 7): with the same k assignment the quarter-warp (2 m x 4 k) again hits 8 different chunks;
+//   * rows / k beyond the matrix are zero-filled by the TMA, so there are no predicates in the loop.
+// One warp (rotating with the slab number) waits for the stage to be drained, posts the byte count on full[s] and
+// issues the boxes; nobody else ever waits on empty[s].
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared.b64 st, [%0], %1;\n}\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
+      "l"(tm), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
+
+template <bool A_KMAJOR, int EPI, int BK_, int STAGES_>
+__global__ void __launch_bounds__(NT3, 1)
+k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int M, int N, int64_t K,
+              int tiles_m, int64_t k_per_split, c128* __restrict__ C, int64_t ldc, double alpha) {
+  constexpr int BK = BK_, STAGES = STAGES_, SS = BK / 8;        // SS sub-slabs of 8 k per stage
+  constexpr int A_SUB = BM * 128, B_SUB = BN * 128;             // bytes of one 8-k sub-slab of A and of B
+  constexpr int A_BYTES = SS * A_SUB, STAGE_BYTES = SS * (A_SUB + B_SUB);
+  extern __shared__ __align__(1024) unsigned char smem[];
+  const uint32_t smem_base = ((uint32_t)__cvta_generic_to_shared(smem) + 1023u) & ~1023u;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp % W3_M, wn = warp / W3_M;
+  int tm, tn;
+  if (A_KMAJOR) { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
+  else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
+  const int m0 = tm * BM, n0 = tn * BN;
+  const int split = blockIdx.y;
+  const int64_t kbeg = (int64_t)split * k_per_split;
+  const int64_t kend = (kbeg + k_per_split < K) ? kbeg + k_per_split : K;
+  const int nkt = (int)((kend - kbeg + BK - 1) / BK);
+
+  const uint32_t bar_full = smem_base + STAGES * STAGE_BYTES, bar_empty = bar_full + STAGES * 8;
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NT3 / 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+
+  // whole warp: post the byte count of slab kt on full[stage] and issue its boxes
+  auto issue_slab = [&](int stage, int kt) {
+    const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES, bar = bar_full + 8 * stage;
+    const int k0 = (int)(kbeg + (int64_t)kt * BK);
+    if (lane == 0) mbar_expect_tx(bar, STAGE_BYTES);
+    __syncwarp();
+    if (A_KMAJOR) {
+      if (lane < SS) tma_load_2d(sa + lane * A_SUB, &tmA, 2 * (k0 + 8 * lane), m0, bar);
+    } else {
+      // box = 8 m (inner) x BK k; m group g goes to sa + g * (BK * 128)
+      if (lane < BM / 8) tma_load_2d(sa + lane * (BK * 128), &tmA, 2 * (m0 + 8 * lane), k0, bar);
+    }
+    if (lane >= 16 && lane < 16 + SS) tma_load_2d(sb + (lane - 16) * B_SUB, &tmB, 2 * (k0 + 8 * (lane - 16)), n0, bar);
+  };
+
+  if (warp == 0) {
+#pragma unroll 1
+    for (int s = 0; s < STAGES - 1; ++s)
+      if (s < nkt) issue_slab(s, s);
+  }
+
+  double t1[4][2][2], t2[4][2][2], t3[4][2][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) { t1[i][j][h] = 0.0; t2[i][j][h] = 0.0; t3[i][j][h] = 0.0; }
+
+  const int frow = lane >> 2, fk = lane & 3;
+  // byte offsets of this thread's fragments for the even k4 steps of a sub-slab (physical k = 2 fk); the odd steps
+  // (k = 2 fk + 1) are one chunk (and, for the M-major A, one k row) further: offset ^ 16 (^ 128), the stage base being
+  // 1024-byte aligned
+  const uint32_t a_off0 = A_KMAJOR ? (uint32_t)((wm * 32 + frow) * 128 + (((2 * fk) ^ frow) * 16))
+                                   : (uint32_t)((wm * 4) * (BK * 128) + (2 * fk) * 128 + ((frow ^ (2 * fk)) * 16));
+  const uint32_t b_off0 = (uint32_t)(A_BYTES + (wn * 16 + frow) * 128 + (((2 * fk) ^ frow) * 16));
+  constexpr uint32_t A_ODD = A_KMAJOR ? 16u : (16u | 128u), B_ODD = 16u;
+
+  for (int kt = 0; kt < nkt; ++kt) {
+    const int stage = kt % STAGES;
+    mbar_wait(bar_full + 8 * stage, (uint32_t)(kt / STAGES) & 1u);
+    const uint32_t st = smem_base + stage * STAGE_BYTES;
+#pragma unroll
+    for (int k4 = 0; k4 < BK / 4; ++k4) {
+      const int ss = k4 >> 1, par = k4 & 1;
+      double2 b[2];
+      double sb[2];
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        b[j] = lds128(((st + b_off0) ^ (par ? B_ODD : 0u)) + (uint32_t)(ss * B_SUB + j * 8 * 128));
+        sb[j] = b[j].x + b[j].y;
+      }
+      if (k4 == 0) {
+        const int nk = kt + STAGES - 1;
+        if (nk < nkt && warp == (kt & 15)) {
+          if (kt >= 1) mbar_wait(bar_empty + 8 * (nk % STAGES), (uint32_t)((kt - 1) / STAGES) & 1u);
+          issue_slab(nk % STAGES, nk);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        // K-major A: sub-slab ss, row block i -> + i*8 rows;  M-major A: m group wm*4 + i, k within the box = 8 ss + ...
+        const uint32_t ao = A_KMAJOR ? (uint32_t)(ss * A_SUB + i * 8 * 128) : (uint32_t)(i * (BK * 128) + ss * 8 * 128);
+        const double2 a = lds128(((st + a_off0) ^ (par ? A_ODD : 0u)) + ao);
+        const double sa = A_KMAJOR ? a.x - a.y : a.x + a.y;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          dmma(t1[i][j][0], t1[i][j][1], a.x, b[j].x);
+          dmma(t2[i][j][0], t2[i][j][1], a.y, b[j].y);
+          dmma(t3[i][j][0], t3[i][j][1], sa, sb[j]);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_empty + 8 * stage);
+  }
+
+  c128* Cout = C;
+  if (EPI == EPI_PARTIAL) Cout += (int64_t)split * ldc * N;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int m = m0 + wm * 32 + i * 8 + frow;
+    if (m >= M) continue;
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int n = n0 + wn * 16 + j * 8 + 2 * fk + h;
+        if (n >= N) continue;
+        const double re = A_KMAJOR ? t1[i][j][h] + t2[i][j][h] : t1[i][j][h] - t2[i][j][h];
+        const double im = A_KMAJOR ? (t3[i][j][h] - t1[i][j][h]) + t2[i][j][h] : (t3[i][j][h] - t1[i][j][h]) - t2[i][j][h];
+        c128* p = Cout + (int64_t)n * ldc + m;
+        if (EPI == EPI_PARTIAL) {
+          *p = cmake(re, im);
+        } else {
+          c128 t = *p;
+          t.x = fma(alpha, re, t.x);
+          t.y = fma(alpha, im, t.y);
+          *p = t;
+        }
+      }
+    }
+  }
+}
+
 // C[m + n*ldc] = scale[m] * sum_s part[s][m + n*M]   (fixed summation order => deterministic)
 __global__ void __launch_bounds__(256) k_splitk_reduce(int M, int N, int nsplit, const c128* __restrict__ part,
                                                        const double* __restrict__ scale, c128* __restrict__ C,
@@ -415,6 +577,9 @@ constexpr int smem_nn() { return STAGES * (A_BYTES_M + B_BYTES); }
 // 3M kernels: CN streams K = npw in slabs of 8 through 4 stages, NN (K = nproj) in slabs of 16 through 3 stages
 // (measured on B200, cfg 3/4: CN 41.3 vs 40.7 TFLOP/s and NN 35.7 vs 38.2 for slabs of 8 vs 16)
 constexpr int CN3_BK = 8, CN3_STAGES = 4, NN3_BK = 16, NN3_STAGES = 3;
+// TMA-fed kernels: CN 8-k slabs x 6 stages (24 KB each), NN 16-k slabs x 4 stages (48 KB each); + 1 KB alignment slack
+constexpr int CNT_BK = 8, CNT_STAGES = 6, NNT_BK = 16, NNT_STAGES = 4;
+constexpr int smem_tma(int bk, int stages) { return stages * (bk / 8) * (BM + BN) * 128 + 2 * stages * 8 + 1024; }
 constexpr int smem_cn3() { return CN3_STAGES * (Tile3<CN3_BK>::A_K + Tile3<CN3_BK>::B_) + 2 * CN3_STAGES * 8; }
 constexpr int smem_nn3() { return NN3_STAGES * (Tile3<NN3_BK>::A_M + Tile3<NN3_BK>::B_) + 2 * NN3_STAGES * 8; }
 constexpr int NUM_SMS = 148;
@@ -427,7 +592,47 @@ static bool use_3m() {
   return v;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_fn() {
+  static const EncodeTiledFn fn = [] {
+    const char* e = getenv("PWH_ZGEMM_NO_TMA");
+    if (e && e[0] == '1') return (EncodeTiledFn) nullptr;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+
+// column-major complex matrix `inner` x `outer` (leading dimension ld) as an FP64 tensor {2 inner, outer};
+// box = 8 complex (128 B, swizzled) x box_outer
+static bool make_map(CUtensorMap* tm, const c128* base, int64_t inner, int64_t outer, int64_t ld, int box_outer) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn || ((uintptr_t)base & 15) || inner < 1 || outer < 1) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)(2 * inner), (cuuint64_t)outer};
+  const cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(c128)};
+  const cuuint32_t box[2] = {16u, (cuuint32_t)box_outer};
+  const cuuint32_t estr[2] = {1u, 1u};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<c128*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 cudaError_t zgemm_init() {
+  {
+    cudaError_t e = cudaFuncSetAttribute(k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem_tma(CNT_BK, CNT_STAGES));
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             smem_tma(NNT_BK, NNT_STAGES));
+    if (e != cudaSuccess) return e;
+  }
   cudaError_t e = cudaFuncSetAttribute(k_zgemm<true, EPI_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_cn());
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_zgemm<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
@@ -489,7 +694,11 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
   c128* part = reinterpret_cast<c128*>(ws);
   {
     ScopedLaunch sl(ST_ZGEMM_CN, st);
-    if (use_3m())
+    CUtensorMap tmA, tmB;
+    if (use_3m() && make_map(&tmA, A, K, M, lda, BM) && make_map(&tmB, B, K, N, ldb, BN))
+      k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES><<<grid, NT3, smem_tma(CNT_BK, CNT_STAGES), st>>>(
+          tmA, tmB, (int)M, (int)N, K, tiles_m, kps, part, M, 0.0);
+    else if (use_3m())
       k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES><<<grid, NT3, smem_cn3(), st>>>(
           (int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
     else
@@ -508,7 +717,11 @@ void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c1
   const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
   dim3 grid(tiles_m * tiles_n, 1);
   ScopedLaunch sl(ST_ZGEMM_NN, st);
-  if (use_3m())
+  CUtensorMap tmA, tmB;
+  if (use_3m() && make_map(&tmA, A, M, K, lda, NNT_BK) && make_map(&tmB, B, K, N, ldb, BN))
+    k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES><<<grid, NT3, smem_tma(NNT_BK, NNT_STAGES), st>>>(
+        tmA, tmB, (int)M, (int)N, K, tiles_m, K, C, ldc, alpha);
+  else if (use_3m())
     k_zgemm3m<false, EPI_ACC, NN3_BK, NN3_STAGES><<<grid, NT3, smem_nn3(), st>>>(
         (int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
   else

@@ -15,6 +15,7 @@
 //   * the x direction is warp-private: a warp owns NYB y-slots at a time and carries them through inverse x,
 //     V_loc multiply and forward x in its own padded buffer with __syncwarp only, so a plane needs 4 CTA barriers;
 //   * V_loc/F is stored as [z-slot][y-batch][q][lane item] so that the multiply reads it fully coalesced.
+#include <cstdlib>
 #include <type_traits>
 
 #include "fft_reg.cuh"
@@ -112,6 +113,12 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
     c128* tw_ = tbuf + warp * (NYB * XP);
     const int x0 = P.x0;
     const double* __restrict__ vz = P.vperm + (int64_t)zslot * ((int64_t)N1 * N2);
+    constexpr int XG = 32 / R1X;               // y-slots pass (b) handles per round: lane = xg * R1X + xk1
+    static_assert(NYB % XG == 0, "pass (b) rounds");
+    const int xk1 = lane % R1X, xg = lane / R1X;
+    c128 xtw[R2X];
+#pragma unroll
+    for (int q = 0; q < R2X; ++q) xtw[q] = twBx[xk1 * (R2X + 1) + q];
     for (int b = warp; b < C::NBATCH; b += C::NW) {
       const int y0 = b * NYB;
       // (a) strided role: radix R1X over x = q R2X + s, twiddle, into the warp buffer at k1 (R2X+1) + s
@@ -128,29 +135,32 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
           v[q] = xq < nxl ? src[xq * YS] : czero();
         }
         Dft<R1X, +1>::run(v);
-        const c128* tw = twAx + s * (R1X + 1);
         c128* dst = tw_ + yb * XP + s;
-        dst[0] = v[0];
 #pragma unroll
-        for (int q = 1; q < R1X; ++q) dst[q * (R2X + 1)] = cmul(v[q], tw[q]);
+        for (int q = 0; q < R1X; ++q) dst[q * (R2X + 1)] = v[q];
       }
       __syncwarp();
-      // (b) contiguous role: radix R2X inverse -> real space, multiply by V_loc/F, radix R2X forward, twiddle
+      // (b) contiguous role: twiddle w^(s k1), radix R2X inverse -> real space, multiply by V_loc/F, radix R2X forward,
+      //     twiddle w^-(s k1).  A lane keeps the same k1 for all its items, so its R2X-1 twiddles live in registers and
+      //     passes (a) and (c) are plain radix-R1X transforms.
       const double* __restrict__ vb = vz + (int64_t)b * (R2X * R1X * NYB);
-      for (int i = lane; i < R1X * NYB; i += 32) {
-        const int k1 = i % R1X, yb = i / R1X;
-        c128* t = tw_ + yb * XP + k1 * (R2X + 1);
-        c128 v[R2X];
+      if (lane < XG * R1X) {
 #pragma unroll
-        for (int q = 0; q < R2X; ++q) v[q] = t[q];
-        Dft<R2X, +1>::run(v);
+        for (int yb = xg; yb < NYB; yb += XG) {
+          const int i = xk1 + R1X * yb;
+          c128* t = tw_ + yb * XP + xk1 * (R2X + 1);
+          c128 v[R2X];
+          v[0] = t[0];
 #pragma unroll
-        for (int q = 0; q < R2X; ++q) v[q] = cscale(vb[q * (R1X * NYB) + i], v[q]);
-        Dft<R2X, -1>::run(v);
-        const c128* tw = twBx + k1 * (R2X + 1);
-        t[0] = v[0];
+          for (int q = 1; q < R2X; ++q) v[q] = cmul(t[q], xtw[q]);
+          Dft<R2X, +1>::run(v);
 #pragma unroll
-        for (int q = 1; q < R2X; ++q) t[q] = cmulc(v[q], tw[q]);
+          for (int q = 0; q < R2X; ++q) v[q] = cscale(vb[q * (R1X * NYB) + i], v[q]);
+          Dft<R2X, -1>::run(v);
+          t[0] = v[0];
+#pragma unroll
+          for (int q = 1; q < R2X; ++q) t[q] = cmulc(v[q], xtw[q]);
+        }
       }
       __syncwarp();
       // (c) strided role: radix R1X forward over k1, keep the touched x-lines
@@ -252,6 +262,7 @@ void v2_launch(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st) {
 using C48 = PC<48, 8, 6, 48, 8, 6, 8, 16>;
 using C96a = PC<96, 12, 8, 96, 12, 8, 16, 4>;
 using C96b = PC<96, 12, 8, 96, 12, 8, 8, 4>;
+using C96c = PC<96, 12, 8, 96, 12, 8, 12, 4>;    // 24 x batches = 2 per warp, 170 registers per thread
 using C120a = PC<120, 15, 8, 120, 15, 8, 10, 4>;
 using C120b = PC<120, 15, 8, 120, 15, 8, 8, 4>;
 using C128a = PC<128, 16, 8, 128, 16, 8, 16, 4>;
@@ -267,6 +278,7 @@ bool v2_dispatch(int variant, F&& f) {
     case 5: f(C120b()); return true;
     case 6: f(C128a()); return true;
     case 7: f(C128b()); return true;
+    case 8: f(C96c()); return true;
     default: return false;
   }
 }
@@ -277,12 +289,18 @@ bool v2_dispatch(int variant, F&& f) {
 // fills the radices, NYB and the variant id of the plan.  Returns false when no specialisation applies.
 bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max) {
   if (n1 != n2) return false;
-  int first = 0, last = -1;
-  if (n1 == 48) { first = last = 1; }
-  else if (n1 == 96) { first = 2; last = 3; }
-  else if (n1 == 120) { first = 4; last = 5; }
-  else if (n1 == 128) { first = 6; last = 7; }
-  for (int var = first; var <= last; ++var) {
+  int order[3] = {0, 0, 0}, norder = 0;
+  if (n1 == 48) { order[norder++] = 1; }
+  else if (n1 == 96) { order[norder++] = 8; order[norder++] = 2; order[norder++] = 3; }
+  else if (n1 == 120) { order[norder++] = 5; order[norder++] = 4; }   // 8 warps measured faster than 10 (12.4 vs 12.9 ms, cfg 5)
+  else if (n1 == 128) { order[norder++] = 6; order[norder++] = 7; }
+  if (const char* e = getenv("PWH_V2_VARIANT")) {   // measurement aid: force one instantiation
+    const int v = atoi(e);
+    for (int oi = 0; oi < norder; ++oi)
+      if (order[oi] == v) { order[0] = v; norder = 1; break; }
+  }
+  for (int oi = 0; oi < norder; ++oi) {
+    const int var = order[oi];
     bool ok = false;
     v2_dispatch(var, [&](auto c) {
       using C = decltype(c);

@@ -597,9 +597,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static EncodeTiledFn encode_fn() {
+  const char* e = getenv("PWH_ZGEMM_NO_TMA");   // read at every call so that the tests can switch kernels
+  if (e && e[0] == '1') return nullptr;
   static const EncodeTiledFn fn = [] {
-    const char* e = getenv("PWH_ZGEMM_NO_TMA");
-    if (e && e[0] == '1') return (EncodeTiledFn) nullptr;
     void* p = nullptr;
     cudaDriverEntryPointQueryResult q;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||

@@ -145,6 +145,21 @@ def test_fallback_kernels_cfg2(gpu, cfg2, monkeypatch, env):
     ham.destroy()
 
 
+def test_zgemm_without_tma(gpu, cfg2, monkeypatch):
+    """The cp.async (LDGSTS) 3M ZGEMM kernels that serve when cuTensorMapEncodeTiled is unavailable or refuses an operand,
+    against the oracle: projector path of apply_h and a ragged Gram product."""
+    monkeypatch.setenv("PWH_ZGEMM_NO_TMA", "1")
+    w = cfg2
+    ham = setup(gpu, w)
+    psi = w.psi[:67]
+    out = gpu.apply_h(ham, to_dev(psi)).cpu().numpy()
+    ref = oracle.apply_h(*ham_args(w), psi)
+    assert relerr(out, ref) <= TOL_H
+    g = gpu.gram(to_dev(psi), to_dev(ref)).cpu().numpy()
+    assert relerr(g, oracle.gram(psi, ref)) <= TOL_H
+    ham.destroy()
+
+
 def test_cfg3_band_subset(gpu):
     """Config 3 (k = 1/4 1/4 1/4, 96^3, 57925 plane waves, 512 projectors) at full N and J on a subset of bands --
     exact, since bands never interact before gram."""

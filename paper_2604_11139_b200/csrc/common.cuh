@@ -105,6 +105,7 @@ struct V2Plan {
   int n1, n2, n3;
   int ncols_pad, nxl;
   int x0;                    // wrapped x of x-line 0: x-line of x is (x - x0) mod n1, touched iff < nxl
+  int zcol;                  // first padding column (>= ncols): zero on input; zcol + 1 takes the stores outside the disc
   int variant;               // which template instantiation
   int r1[2], r2[2], nyb;     // x, y radices and y-slots per warp batch of that instantiation
   const int2* yrow;          // [n2] per wrapped y: .x = first column - xlmin, .y = xlmin | (count << 16)

@@ -37,7 +37,7 @@ struct PC {
   static constexpr int TWA_Y = R2Y * (R1Y + 1), TWB_Y = R1Y * (R2Y + 1);
   static constexpr int NBATCH = N2 / NYB;
   static size_t smem_bytes(int nxl) {
-    return sizeof(c128) * ((size_t)nxl * YS + (size_t)NW * NYB * XP + TWA_X + TWB_X + TWA_Y + TWB_Y) + sizeof(int2) * N2;
+    return sizeof(c128) * ((size_t)(nxl + 2) * YS + (size_t)NW * NYB * XP + TWA_X + TWB_X + TWA_Y + TWB_Y) + sizeof(int2) * N2;
   }
 };
 
@@ -49,8 +49,9 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
   constexpr int NT = C::NT, YS = C::YS, XP = C::XP, NYB = C::NYB;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nxl = P.nxl;
-  c128* half = reinterpret_cast<c128*>(smem_raw);            // [nxl][YS]
-  c128* tbuf = half + nxl * YS;                              // [NW][NYB][XP]
+  c128* half = reinterpret_cast<c128*>(smem_raw);            // [nxl + 2][YS]: line nxl stays zero (read for the
+                                                             // untouched x-lines), line nxl + 1 takes the stores to them
+  c128* tbuf = half + (nxl + 2) * YS;                        // [NW][NYB][XP]
   c128* twAx = tbuf + C::NW * NYB * XP;                      // [R2X][R1X+1]  w^(s k1)
   c128* twBx = twAx + C::TWA_X;                              // [R1X][R2X+1]  w^(s k1)
   c128* twAy = twBx + C::TWB_X;
@@ -64,9 +65,11 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
   for (int i = tid; i < C::TWA_Y; i += NT) twAy[i] = P.twA[1][i];
   for (int i = tid; i < C::TWB_Y; i += NT) twBy[i] = P.twB[1][i];
   for (int i = tid; i < N2; i += NT) yrow[i] = P.yrow[i];
+  for (int i = tid; i < YS; i += NT) half[nxl * YS + i] = czero();
   __syncthreads();
 
   c128* __restrict__ plane = colbuf + ((int64_t)band * P.n3 + zslot) * P.ncols_pad;
+  const int zcol = P.zcol;
 
   // ---- y1: inverse y, strided role (radix R1Y over y = q R2Y + s), input straight from the disc in global memory
   {
@@ -80,7 +83,7 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
       for (int q = 0; q < R1Y; ++q) {
         const int2 row = yr[q * R2Y];
         const uint32_t d = l - (uint32_t)(row.y & 0xffff);
-        v[q] = d < (uint32_t)(row.y >> 16) ? plane[row.x + (int)l] : czero();
+        v[q] = plane[d < (uint32_t)(row.y >> 16) ? row.x + (int)l : zcol];   // zcol: a padding column, always zero
       }
       Dft<R1Y, +1>::run(v);
       const c128* tw = twAy + s * (R1Y + 1);
@@ -132,7 +135,7 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
         for (int q = 0; q < R1X; ++q) {
           int xq = xl + q * R2X;
           if (xq >= N1) xq -= N1;
-          v[q] = xq < nxl ? src[xq * YS] : czero();
+          v[q] = src[(xq < nxl ? xq : nxl) * YS];
         }
         Dft<R1X, +1>::run(v);
         c128* dst = tw_ + yb * XP + s;
@@ -178,7 +181,7 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
         for (int q = 0; q < R1X; ++q) {
           int xq = xl + q * R2X;
           if (xq >= N1) xq -= N1;
-          if (xq < nxl) dst[xq * YS] = v[q];
+          dst[(xq < nxl ? xq : nxl + 1) * YS] = v[q];
         }
       }
       __syncwarp();
@@ -220,7 +223,7 @@ __global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __re
       for (int q = 0; q < R1Y; ++q) {
         const int2 row = yr[q * R2Y];
         const uint32_t d = l - (uint32_t)(row.y & 0xffff);
-        if (d < (uint32_t)(row.y >> 16)) plane[row.x + (int)l] = v[q];
+        plane[d < (uint32_t)(row.y >> 16) ? row.x + (int)l : zcol + 1] = v[q];   // zcol + 1: padding column nobody reads
       }
     }
   }

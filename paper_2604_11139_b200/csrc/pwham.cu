@@ -337,7 +337,7 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   lp.ncols = ncols;
   lp.nxl = nxl;
   lp.colgrp = h->fast ? 32 : 16;
-  lp.ngrp = (ncols + lp.colgrp - 1) / lp.colgrp;
+  lp.ngrp = (ncols + 2 + lp.colgrp - 1) / lp.colgrp;   // at least two padding columns (kv2_plane: a zero one and a dump)
   lp.ncols_pad = lp.ngrp * lp.colgrp;
   lp.zstride = n3 | 1;
   lp.ystride = n2 | 1;
@@ -450,6 +450,7 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     if (ok) ok = v2_select(vp, n1, n2, nxl, (size_t)smem_max);
     if (ok) {
       vp.n1 = n1; vp.n2 = n2; vp.n3 = n3; vp.ncols_pad = lp.ncols_pad; vp.nxl = nxl; vp.x0 = x_of_xl[0];
+      vp.zcol = ncols;
       vp.div_nxl = lp.div_nxl;
       if ((rc = upload(h, yrow, &vp.yrow, st))) return rc;
       const long double PI = 3.14159265358979323846264338327950288L;

@@ -194,6 +194,22 @@ def run_reference(args):
 # ----------------------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ----------------------------------------------------------------------------------------------------------------
+def max_over_ranks(dist, ms: float, device) -> float:
+    """Device-timed milliseconds of the slowest replica (the path has no collective: every rank runs the whole step on its
+    own GPU); `dist` is torch.distributed or None for a single process."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, nband: int, napps: int, ms_step: float) -> float:
+    """band H.psi applications per second of all replicas together (weak scaling: each rank does the full workload)."""
+    return world * nband * napps / (ms_step * 1e-3)
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -266,15 +282,12 @@ def run_ours(args):
     barrier()
     launches = binding.launch_count() - n0
     ms_total = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(dist, ms_total, dev)
     clocks = sampler.stop() if rank == 0 else {}
     ms_step = ms_total / args.steps
     nblocks = -(-M // blk)
     filter_ms_block = sum(a.elapsed_time(b) for a, b in filter_events) / (args.steps * nblocks)
-    value = world * M * napps / (ms_step * 1e-3)
+    value = whole_job_value(world, M, napps, ms_step)
 
     if rank != 0:
         if dist is not None:
@@ -316,7 +329,7 @@ def run_ours(args):
     fp64_nominal = 148 * 128 * 1.965e9 * 1e-12          # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s
     if zg_ms >= loc_ms and zg_ms > 0:
         ach = zg_flops / (zg_ms * 1e-3) * 1e-12
-        roofline = {"bound": "tensor", "kernel": "k_zgemm (DMMA m8n8k4.f64; CN + NN instantiations)",
+        roofline = {"bound": "tensor", "kernel": "k_zgemm3m_tma (3M complex product on DMMA m8n8k4.f64, TMA-fed; CN + NN instantiations)",
                     "achieved": ach, "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma,
                     "peak_source": "pwh_probe_fp64_tensor_peak, register-resident DMMA loop measured in this run "
                                    f"(nominal 148 SM x 128 flop/clk x 1.965 GHz = {fp64_nominal:.1f})",
@@ -325,7 +338,7 @@ def run_ours(args):
                     "traffic": PROFILED_TRAFFIC.get(("zgemm", args.cfg))}
     else:
         ach = loc_bytes / (loc_ms * 1e-3) * 1e-9
-        roofline = {"bound": "hbm", "kernel": "k_scatter_zinv + k_plane + k_zfwd_gather (local potential + recurrence)",
+        roofline = {"bound": "hbm", "kernel": "kz_scatter_zinv + kv2_plane + kz_zfwd_gather (local potential + recurrence)",
                     "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "peak_source": hbm_src,
                     "traffic": PROFILED_TRAFFIC.get(("local", args.cfg))}
     local_roof = {"ms_per_step": loc_ms / args.steps,
@@ -389,7 +402,11 @@ def run_ours(args):
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full` captures
 # under profiles/ -- filled in per round; None where no capture exists for that config.
-PROFILED_TRAFFIC = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full` captures
+# (profiles/r01e_cfg4.md: CN 6.35 GB, NN 6.82 GB, cold cache; profiles/r01c_cfg3_ncu_full.md for cfg 3), averaged over
+# the CN and NN launches like `achieved`
+PROFILED_TRAFFIC = {("zgemm", 4): 0.5 * (6.231801e9 + 0.120861e9 + 4.602920e9 + 2.220826e9),
+                    ("zgemm", 3): 0.5 * (1.032454e9 + 0.081808e9 + 0.953950e9 + 0.433480e9)}
 
 
 def main():

@@ -107,7 +107,10 @@ int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny
  * k-point and SCF step, Algorithm 3).  All pointers below marked HOST are host memory (pinned
  * memory gives asynchronous copies; pageable memory works).  Device staging buffers are allocated on first use,
  * cached in the handle and freed by pwh_ham_destroy.  Each call copies its inputs to the device, runs the same
- * kernels as the device entry points, copies the result back and synchronises.
+ * kernels as the device entry points, copies the result back and synchronises.  The filtering entry points move Psi
+ * in chunks of bands (the column blocks, or quarters of a single block of >= 512 bands) on two internal copy streams,
+ * so that the copies of the neighbouring chunks run under the filter of the current one (bands never interact before
+ * the Gram product); every band still goes through exactly the same kernels.
  *
  * pwh_apply_h_host     hpsi_host = H psi_host.
  * pwh_cheb_filter_host psi_host <- p_m(H) psi_host, bands processed in column blocks of `block` (<= 0: all at once).

@@ -94,6 +94,9 @@ struct pwh_ham {
   void* st_g = nullptr;
   void* st_ws = nullptr;
   size_t st_psi_bytes = 0, st_hpsi_bytes = 0, st_g_bytes = 0, st_ws_bytes = 0;
+  // copy streams and events of the pipelined host entry points
+  cudaStream_t cs_in = nullptr, cs_out = nullptr;
+  std::vector<cudaEvent_t> evs;
 };
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -228,6 +231,9 @@ extern "C" int pwh_ham_destroy(pwh_ham* h) {
   if (h->st_hpsi) cudaFree(h->st_hpsi);
   if (h->st_g) cudaFree(h->st_g);
   if (h->st_ws) cudaFree(h->st_ws);
+  if (h->cs_in) cudaStreamDestroy(h->cs_in);
+  if (h->cs_out) cudaStreamDestroy(h->cs_out);
+  for (cudaEvent_t e : h->evs) cudaEventDestroy(e);
   delete h;
   return PWH_OK;
 }
@@ -786,6 +792,56 @@ static int filter_blocks(pwh_ham* h, int64_t nband, int64_t block, c128* psi_dev
   return PWH_OK;
 }
 
+// The host entry points move Psi in chunks of bands on two copy streams so that the host->device copy of chunk i+1 and
+// the device->host copy of chunk i-1 run under the filter of chunk i (bands never interact before gram, PAPER.md:117,
+// 224): the column blocks of `block` bands when there are several, otherwise quarters of the block.
+static int64_t pipeline_chunk(int64_t nband, int64_t block) {
+  if (block <= 0 || block > nband) block = nband;
+  if (block < nband || nband < 512) return block;
+  return ((nband + 3) / 4 + 63) / 64 * 64;
+}
+
+static int pipeline_init(pwh_ham* h, size_t nevents) {
+  if (!h->cs_in) CUDA_TRY(cudaStreamCreateWithFlags(&h->cs_in, cudaStreamNonBlocking));
+  if (!h->cs_out) CUDA_TRY(cudaStreamCreateWithFlags(&h->cs_out, cudaStreamNonBlocking));
+  while (h->evs.size() < nevents) {
+    cudaEvent_t e;
+    CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    h->evs.push_back(e);
+  }
+  return PWH_OK;
+}
+
+// H2D of all chunks on cs_in, filter of chunk c on `st` as soon as it has landed, D2H of the filtered chunk on cs_out
+static int filter_pipelined(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree, double a,
+                            double b, double a0, cudaStream_t st) {
+  const int64_t chunk = pipeline_chunk(nband, block);
+  const int64_t nchunks = (nband + chunk - 1) / chunk;
+  const size_t row = (size_t)h->npw * sizeof(c128);
+  int rc;
+  if ((rc = pipeline_init(h, (size_t)(2 * nchunks + 1)))) return rc;
+  c128* dev = (c128*)h->st_psi;
+  CUDA_TRY(cudaEventRecord(h->evs[0], st));                       // earlier work on `st` may still use the staging buffer
+  CUDA_TRY(cudaStreamWaitEvent(h->cs_in, h->evs[0], 0));
+  for (int64_t c = 0; c < nchunks; ++c) {
+    const int64_t b0 = c * chunk, nb = std::min(chunk, nband - b0);
+    CUDA_TRY(cudaMemcpy2DAsync(dev + b0 * h->npw, row, (const c128*)psi_host + b0 * ld, (size_t)ld * sizeof(c128), row,
+                               (size_t)nb, cudaMemcpyHostToDevice, h->cs_in));
+    CUDA_TRY(cudaEventRecord(h->evs[1 + c], h->cs_in));
+  }
+  for (int64_t c = 0; c < nchunks; ++c) {
+    const int64_t b0 = c * chunk, nb = std::min(chunk, nband - b0);
+    CUDA_TRY(cudaStreamWaitEvent(st, h->evs[1 + c], 0));
+    if ((rc = filter_blocks(h, nb, std::min<int64_t>(block > 0 ? block : nb, nb), dev + b0 * h->npw, h->npw, degree, a, b, a0, st)))
+      return rc;
+    CUDA_TRY(cudaEventRecord(h->evs[1 + nchunks + c], st));
+    CUDA_TRY(cudaStreamWaitEvent(h->cs_out, h->evs[1 + nchunks + c], 0));
+    CUDA_TRY(cudaMemcpy2DAsync((c128*)psi_host + b0 * ld, (size_t)ld * sizeof(c128), dev + b0 * h->npw, row, row, (size_t)nb,
+                               cudaMemcpyDeviceToHost, h->cs_out));
+  }
+  return PWH_OK;
+}
+
 extern "C" int pwh_cheb_filter_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
                                     double a, double b, double a0, void* stream) {
   if (!h) return fail(PWH_EINVAL, "handle is null");
@@ -796,14 +852,13 @@ extern "C" int pwh_cheb_filter_host(pwh_ham* h, int64_t nband, int64_t block, pw
   if (ld < h->npw) return fail(PWH_EINVAL, "ld < npw");
   cudaStream_t st = (cudaStream_t)stream;
   if (block <= 0 || block > nband) block = nband;
-  const size_t blk = (size_t)h->npw * nband * sizeof(c128), row = (size_t)h->npw * sizeof(c128);
+  const size_t blk = (size_t)h->npw * nband * sizeof(c128);
   int rc;
   if ((rc = ensure(&h->st_psi, &h->st_psi_bytes, blk))) return rc;
-  if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, pwh_workspace_bytes(h, block)))) return rc;
-  CUDA_TRY(cudaMemcpy2DAsync(h->st_psi, row, psi_host, (size_t)ld * sizeof(c128), row, nband, cudaMemcpyHostToDevice, st));
-  if ((rc = filter_blocks(h, nband, block, (c128*)h->st_psi, h->npw, degree, a, b, a0, st))) return rc;
-  CUDA_TRY(cudaMemcpy2DAsync(psi_host, (size_t)ld * sizeof(c128), h->st_psi, row, row, nband, cudaMemcpyDeviceToHost, st));
+  if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, pwh_workspace_bytes(h, std::min(block, pipeline_chunk(nband, block)))))) return rc;
+  if ((rc = filter_pipelined(h, nband, block, psi_host, ld, degree, a, b, a0, st))) return rc;
   CUDA_TRY(cudaStreamSynchronize(st));
+  CUDA_TRY(cudaStreamSynchronize(h->cs_out));
   return PWH_OK;
 }
 
@@ -826,8 +881,7 @@ extern "C" int pwh_sweep_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128
   if ((rc = ensure(&h->st_hpsi, &h->st_hpsi_bytes, blk))) return rc;
   if ((rc = ensure(&h->st_g, &h->st_g_bytes, gbytes))) return rc;
   if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, wsb))) return rc;
-  CUDA_TRY(cudaMemcpy2DAsync(h->st_psi, row, psi_host, (size_t)ld * sizeof(c128), row, nband, cudaMemcpyHostToDevice, st));
-  if ((rc = filter_blocks(h, nband, block, (c128*)h->st_psi, h->npw, degree, a, b, a0, st))) return rc;
+  if ((rc = filter_pipelined(h, nband, block, psi_host, ld, degree, a, b, a0, st))) return rc;
   for (int64_t b0 = 0; b0 < nband; b0 += block) {
     const int64_t nb = std::min(block, nband - b0);
     rc = pwh_apply_h(h, nb, (const pwh_c128*)((c128*)h->st_psi + b0 * h->npw), h->npw,
@@ -837,12 +891,12 @@ extern "C" int pwh_sweep_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128
   rc = pwh_gram(h->npw, nband, (const pwh_c128*)h->st_psi, h->npw, nband, (const pwh_c128*)h->st_hpsi, h->npw,
                 (pwh_c128*)h->st_g, nband, h->st_ws, h->st_ws_bytes, st);
   if (rc) return rc;
-  CUDA_TRY(cudaMemcpy2DAsync(psi_host, (size_t)ld * sizeof(c128), h->st_psi, row, row, nband, cudaMemcpyDeviceToHost, st));
   if (hpsi_host)
     CUDA_TRY(cudaMemcpy2DAsync(hpsi_host, (size_t)ldh * sizeof(c128), h->st_hpsi, row, row, nband, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaMemcpy2DAsync(G_host, (size_t)ldg * sizeof(c128), h->st_g, (size_t)nband * sizeof(c128),
                              (size_t)nband * sizeof(c128), nband, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
+  CUDA_TRY(cudaStreamSynchronize(h->cs_out));
   return PWH_OK;
 }
 

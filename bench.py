@@ -335,6 +335,10 @@ def run_ours(args):
                                    f"(nominal 148 SM x 128 flop/clk x 1.965 GHz = {fp64_nominal:.1f})",
                     "frac_of_nominal": ach / fp64_nominal,
                     "flops_per_launch": zg_flops / max(zg_n, 1), "ms_per_launch": zg_ms / max(zg_n, 1),
+                    "pipe_busy_frac": 0.75 * ach / peak_dmma,
+                    "note": "flops counted as 8mnk per complex GEMM (SURVEY.md 8d-4) while the 3M product spends 6mnk on "
+                            "the pipe, so frac can exceed 1; pipe_busy_frac = 0.75 x frac is the share of the DMMA peak "
+                            "actually occupied (ncu pipe_tensor: 90.4 % CN / 85.5 % NN, profiles/r01e_cfg4.md)",
                     "traffic": PROFILED_TRAFFIC.get(("zgemm", args.cfg))}
     else:
         ach = loc_bytes / (loc_ms * 1e-3) * 1e-9

@@ -5,7 +5,7 @@
 //
 // Same arithmetic as kf_plane in local_fast.cu (two-pass register-resident transforms, n = r1 * r2, real-space data in
 // "slot" order, V_loc stored once in the order the kernel reads it), re-organised around what the ncu capture of
-// kf_plane showed (profiles/r01b_*): 59 % of its instructions were integer/address work of the generic radix dispatch,
+// kf_plane showed (profiles/r01a_*): 59 % of its instructions were integer/address work of the generic radix dispatch,
 // its code did not fit the instruction cache, and every pass ended in a CTA-wide barrier with 16 warps resident.
 //   * the box sides and radices are template parameters: every shared-memory access is base + immediate offset;
 //   * the disc is read from and written to global memory directly by the first / last y pass (per-row range tables,
@@ -15,6 +15,11 @@
 //   * the x direction is warp-private: a warp owns NYB y-slots at a time and carries them through inverse x,
 //     V_loc multiply and forward x in its own padded buffer with __syncwarp only, so a plane needs 4 CTA barriers;
 //   * V_loc/F is stored as [z-slot][y-batch][q][lane item] so that the multiply reads it fully coalesced.
+//   * the inter-pass twiddles of the x direction are applied on both sides of the contiguous-role pass, where a lane keeps
+//     the same k1 for all its items: they live in registers, and the strided-role passes are plain radix-r1 transforms;
+//   * no load or store is predicated: x-lines outside the sphere are read from a zero line and stored to a dump line of
+//     the half-plane, rows outside the disc are read from a zero padding column and stored to a dump padding column
+//     (16 predicates per radix-16 item had to be packed into a register and unpacked again).
 #include <cstdlib>
 #include <type_traits>
 

@@ -4,9 +4,11 @@
 //                                        Rayleigh-Ritz Gram product Psi^H (H Psi), split over K
 //   "NN":  C += alpha A B with K = nproj -> P . (D . P^H psi) accumulated onto the recurrence term
 // tcgen05 has no f64 kind, so FP64 contractions on sm_100a are warp-level DMMA with register accumulators
-// (measured on B200: DMMA.8x8x4 peak 37.1 TFLOP/s == DFMA peak).  One complex product is four real DMMAs on
-// split re/im fragments; operands are staged gmem -> smem with a 4-stage cp.async pipeline in padded layouts
-// that make every 16-byte fragment load conflict-free.
+// (measured on B200: DMMA.8x8x4 peak 37.1 TFLOP/s == DFMA peak).  Three generations of the kernel live here:
+//   k_zgemm3m_tma  (default)  3M complex product, operand slabs by TMA with 128-byte swizzle, mbarrier hand-over
+//   k_zgemm3m      (fallback) 3M, slabs by cp.async into padded layouts, same mbarrier hand-over  (PWH_ZGEMM_NO_TMA=1)
+//   k_zgemm        (reference) four real DMMAs per complex product, cp.async + __syncthreads     (PWH_ZGEMM_4M=1)
+// Every shared-memory layout is chosen so that the 16-byte fragment loads of a quarter-warp are conflict-free.
 #include <cuda.h>
 
 #include <algorithm>
@@ -25,7 +27,7 @@ namespace {
 #define PWH_STAGES 4
 #endif
 constexpr int BM = 128, BN = 64, BK = PWH_BK, STAGES = PWH_STAGES, NT = 256;
-constexpr int WARPS_M = 4, WARPS_N = 2;               // 8 warps, warp tile 32 x 32 complex
+constexpr int WARPS_M = 4;                            // k_zgemm: 4 x 2 warps, warp tile 32 x 32 complex
 constexpr int KROW = BK * 16 + 64;                     // bytes per row of a K-major tile (== 64 mod 128)
 constexpr int MROW = BM * 16 + 32;                     // bytes per k-row of an M-major A tile (== 32 mod 128)
 constexpr int A_BYTES_K = BM * KROW;                   // 24576
@@ -221,7 +223,7 @@ k_zgemm(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* _
 // was no faster (NN 37.5 vs 38.1), so one CTA computes one tile.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int NT3 = 512;
-constexpr int W3_M = 4, W3_N = 4;                      // warp grid; warp tile 32 x 16
+constexpr int W3_M = 4;                                // 4 x 4 warps; warp tile 32 x 16
 
 template <int BK_>
 struct Tile3 {

@@ -30,12 +30,13 @@ namespace pwh {
 
 namespace {
 
-template <int N1_, int R1X_, int R2X_, int N2_, int R1Y_, int R2Y_, int NW_, int NYB_>
+template <int N1_, int R1X_, int R2X_, int N2_, int R1Y_, int R2Y_, int NW_, int NYB_, int MINB_ = 1>
 struct PC {
   static constexpr int N1 = N1_, R1X = R1X_, R2X = R2X_, N2 = N2_, R1Y = R1Y_, R2Y = R2Y_, NW = NW_, NYB = NYB_;
   static_assert(R1X * R2X == N1 && R1Y * R2Y == N2, "axis factorisation");
   static_assert(N2 % NYB == 0, "y batches");
   static constexpr int NT = NW * 32;
+  static constexpr int MINB = MINB_;                 // CTAs per SM the register budget is capped for
   static constexpr int YS = N2 | 1;                  // odd line stride of the half-plane (elements)
   static constexpr int XP = R1X * (R2X + 1);         // padded length of one x-line in a warp buffer
   static constexpr int TWA_X = R2X * (R1X + 1), TWB_X = R1X * (R2X + 1);
@@ -49,7 +50,7 @@ struct PC {
 __device__ __forceinline__ c128 czero() { return cmake(0.0, 0.0); }
 
 template <class C>
-__global__ void __launch_bounds__(C::NT, 1) kv2_plane(const V2Plan P, c128* __restrict__ colbuf) {
+__global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128* __restrict__ colbuf) {
   constexpr int N1 = C::N1, R1X = C::R1X, R2X = C::R2X, N2 = C::N2, R1Y = C::R1Y, R2Y = C::R2Y;
   constexpr int NT = C::NT, YS = C::YS, XP = C::XP, NYB = C::NYB;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -268,8 +269,10 @@ void v2_launch(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st) {
 
 // the specialisations: box side -> (r1, r2) and the (warps, y-slots per warp batch) variants tried in this order
 using C48 = PC<48, 8, 6, 48, 8, 6, 8, 16>;
+using C48b = PC<48, 8, 6, 48, 8, 6, 4, 8, 4>;     // small plane: 4 CTAs of 4 warps per SM instead of one of 8
 using C96a = PC<96, 12, 8, 96, 12, 8, 16, 4>;
 using C96b = PC<96, 12, 8, 96, 12, 8, 8, 4>;
+using C96d = PC<96, 12, 8, 96, 12, 8, 4, 4, 2>;    // two CTAs of 4 warps per SM (113 KB each): independent phases overlap
 using C96c = PC<96, 12, 8, 96, 12, 8, 12, 4>;    // 24 x batches = 2 per warp, 170 registers per thread
 using C120a = PC<120, 15, 8, 120, 15, 8, 10, 4>;
 using C120b = PC<120, 15, 8, 120, 15, 8, 8, 4>;
@@ -287,6 +290,8 @@ bool v2_dispatch(int variant, F&& f) {
     case 6: f(C128a()); return true;
     case 7: f(C128b()); return true;
     case 8: f(C96c()); return true;
+    case 9: f(C48b()); return true;
+    case 10: f(C96d()); return true;
     default: return false;
   }
 }
@@ -297,9 +302,9 @@ bool v2_dispatch(int variant, F&& f) {
 // fills the radices, NYB and the variant id of the plan.  Returns false when no specialisation applies.
 bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max) {
   if (n1 != n2) return false;
-  int order[3] = {0, 0, 0}, norder = 0;
-  if (n1 == 48) { order[norder++] = 1; }
-  else if (n1 == 96) { order[norder++] = 8; order[norder++] = 2; order[norder++] = 3; }
+  int order[4] = {0, 0, 0, 0}, norder = 0;
+  if (n1 == 48) { order[norder++] = 9; order[norder++] = 1; }
+  else if (n1 == 96) { order[norder++] = 10; order[norder++] = 8; order[norder++] = 2; }
   else if (n1 == 120) { order[norder++] = 5; order[norder++] = 4; }   // 8 warps measured faster than 10 (12.4 vs 12.9 ms, cfg 5)
   else if (n1 == 128) { order[norder++] = 6; order[norder++] = 7; }
   if (const char* e = getenv("PWH_V2_VARIANT")) {   // measurement aid: force one instantiation

@@ -666,9 +666,9 @@ cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float
 
 int zgemm_cn_splits(int64_t M, int64_t N, int64_t K) {
   // Split K so that tiles * splits fills whole waves of the 148 SMs (one CTA per SM): among the candidates with at
-  // most 16 waves and at least 32 k-slabs per split, take the fewest splits within 1 % of the best wave efficiency.
+  // most 16 waves and at least 8 k-slabs per split, take the fewest splits within 1 % of the best wave efficiency.
   const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
-  const int64_t max_split = std::max<int64_t>(1, K / (32 * BK));
+  const int64_t max_split = std::max<int64_t>(1, K / (8 * BK));   // at least 8 k-slabs per split (small problems: one wave of short CTAs)
   int best = 1;
   double best_eff = 0.0;
   for (int64_t s = 1; s <= max_split; ++s) {

@@ -41,9 +41,11 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--cfg", type=int, default=int(os.environ.get("PWH_BENCH_CFG", "4")), choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--cfg", type=int, default=int(os.environ.get("PWH_BENCH_CFG", "5")), choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config; default 5 = the largest single-GPU workload (the metric names no config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--profile-steps", type=int, default=2, help="steps of the per-kernel event-timed pass (after the timed region)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU seconds of the oracle sample")
     return ap.parse_args()
@@ -138,25 +140,37 @@ def stage_model(w, info):
     }
 
 
+def oracle_sample(oracle, w, nb: int, light: bool = False):
+    """One bounded sample of the step on the CPU oracle, on the first `nb` bands.  Full: a degree-2 Chebyshev filter (2 H
+    applications and the three-term recurrence), H.Psi and the Gram product = 3 H applications per band.  Light (the
+    --impl reference arm, which repeats it K + W times): a degree-1 filter and the Gram product = 1 H application per
+    band.  Returns (seconds, H applications per band)."""
+    args = (w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, w.proj, w.dij)
+    t0 = time.perf_counter()
+    if light:
+        y = oracle.cheb_filter(*args, w.psi[:nb], 1, w.a, w.b, w.a0)
+        oracle.gram(w.psi[:nb], y)
+        return time.perf_counter() - t0, 1
+    y = oracle.cheb_filter(*args, w.psi[:nb], 2, w.a, w.b, w.a0)
+    hy = oracle.apply_h(*args, y)
+    oracle.gram(y, hy)
+    return time.perf_counter() - t0, 3
+
+
 def cpu_baseline(w, target_s: float):
-    """The oracle as it stands on the host cores: H applications on a bounded sample of bands."""
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
     import oracle
     cores = oracle.n_threads()
-    args = (w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, w.proj, w.dij)
     nb = min(w.psi.shape[0], cores)
-    t0 = time.perf_counter()
-    oracle.apply_h(*args, w.psi[:nb])
-    t = time.perf_counter() - t0
+    t, apps = oracle_sample(oracle, w, nb)
     if t < target_s / 3 and nb < w.psi.shape[0]:
         per = t / max(1, -(-nb // cores))                       # seconds per wave of `cores` bands
         waves = max(1, int(target_s / max(per, 1e-6)))
         nb = min(w.psi.shape[0], waves * cores)
-        t0 = time.perf_counter()
-        oracle.apply_h(*args, w.psi[:nb])
-        t = time.perf_counter() - t0
-    return {"value": nb / t, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"oracle.apply_h (C, -O2, OpenMP over bands) on the first {nb} bands of the same workload, "
-                      f"1 H application each, {t:.1f} s wall"}
+        t, apps = oracle_sample(oracle, w, nb)
+    return {"value": nb * apps / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"oracle (C, -O2, OpenMP over bands) on the first {nb} bands of the same workload: degree-2 Chebyshev "
+                      f"filter + H.Psi + Gram {nb}x{nb} = {apps} H applications per band, {t:.1f} s wall"}
 
 
 def run_reference(args):
@@ -170,17 +184,18 @@ def run_reference(args):
     nb = min(spec.nband, cores)
     w = synth.make_workload(args.cfg, nband=nb, qr="none")
     w.spec = __import__("dataclasses").replace(w.spec, block=spec.block)
-    hargs = (w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, w.proj, w.dij)
+    # bounded: one step = one H application on at most `cores` bands (one band per core), so that the whole
+    # --steps K --warmup W run ends within a few minutes even at cfg 5 (about 6 s per step on 16 cores)
+    apps = 1
     for _ in range(args.warmup):
-        oracle.apply_h(*hargs, w.psi)
-    t0 = time.perf_counter()
+        oracle_sample(oracle, w, nb, light=True)
+    t = 0.0
     for _ in range(args.steps):
-        oracle.apply_h(*hargs, w.psi)
-    t = time.perf_counter() - t0
-    value = nb * args.steps / t
-    sample = (f"each step = oracle.apply_h on {nb} bands x 1 H application of the same config "
-              f"(bounded sample of its {spec.nband} bands x {apps_per_band(spec)} applications)")
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        t += oracle_sample(oracle, w, nb, light=True)[0]
+    value = nb * apps * args.steps / t
+    sample = (f"each step = the oracle on {nb} bands: degree-1 Chebyshev filter (1 H application + the first recurrence step) "
+              f"+ Gram {nb}x{nb} (bounded sample of the config's {spec.nband} bands x {apps_per_band(spec)} applications)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(w).replace(f"nband={nb}", f"nband={spec.nband}").replace(f"Gram {nb}x{nb}", f"Gram {spec.nband}x{spec.nband}"), "sample": sample},
@@ -263,7 +278,7 @@ def run_ours(args):
         if spec.with_gram:
             for b0 in range(0, M, blk):
                 binding.apply_h(ham, psi[b0:b0 + blk], hpsi[b0:b0 + blk])
-            return binding.gram(psi, hpsi)
+            return binding.gram(psi, hpsi, hermitian=True)     # Psi^H (H Psi) is Hermitian
         return None
 
     for _ in range(max(args.warmup, 0)):
@@ -296,14 +311,15 @@ def run_ours(args):
         return 0
 
     # ---- per-kernel times: a second pass of the same K steps with one CUDA-event pair around every launch
+    psteps = max(1, min(args.steps, args.profile_steps))
     binding.profile_begin()
     pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     pe0.record()
-    for _ in range(args.steps):
+    for _ in range(psteps):
         step()
     pe1.record()
     stages = binding.profile_end()
-    ms_step_profiled = pe0.elapsed_time(pe1) / args.steps
+    ms_step_profiled = pe0.elapsed_time(pe1) / psteps
     peak_dmma = binding.probe_fp64_tensor_peak(20000, dev)
 
     peaks = {}
@@ -315,42 +331,56 @@ def run_ours(args):
     hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
 
     mod = stage_model(w, info)
-    band_apps = M * napps * args.steps
-    gram_flops = 8.0 * N * M * M * args.steps if spec.with_gram else 0.0
+    band_apps = M * napps * psteps                       # of the per-kernel pass the stage times come from
+    # Gram Psi^H (H Psi): 8 N M^2 flops by definition (4M convention); the Hermitian kernel computes only the 128 x 64 tiles
+    # with floor(m/128) <= floor(n/128)
+    tiles_m, tiles_n = -(-M // 128), -(-M // 64)
+    herm_tiles = sum(min(tiles_m, tn // 2 + 1) for tn in range(tiles_n))
+    gram_def = 8.0 * N * M * M * psteps if spec.with_gram else 0.0
+    gram_exec = 6.0 * N * herm_tiles * 128 * 64 * psteps if spec.with_gram else 0.0
     zg_ms = stages.get("zgemm_cn", (0.0, 0))[0] + stages.get("zgemm_nn", (0.0, 0))[0]
     zg_n = stages.get("zgemm_cn", (0.0, 0))[1] + stages.get("zgemm_nn", (0.0, 0))[1]
-    zg_flops = mod["zgemm_flops"] * band_apps + gram_flops
+    zg_def = mod["zgemm_flops"] * band_apps + gram_def              # 8 m n k per complex GEMM
+    zg_exec = 0.75 * mod["zgemm_flops"] * band_apps + gram_exec     # what the 3M kernels put on the DMMA pipe: 6 m n k
     loc_ms = sum(stages.get(k, (0.0, 0))[0] for k in ("scatter_zinv", "plane", "zfwd_gather"))
+    loc_n = sum(stages.get(k, (0.0, 0))[1] for k in ("scatter_zinv", "plane", "zfwd_gather"))
     loc_bytes = (mod["local_bytes"] + mod["recurrence_bytes"]) * band_apps
     loc_flops = mod["local_flops"] * band_apps
     all_ms = sum(v[0] for v in stages.values())
-    stage_out = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps,
+    stage_out = {k: {"ms_per_step": v[0] / psteps, "launches_per_step": v[1] / psteps,
                      "share": v[0] / all_ms if all_ms else None} for k, v in stages.items()}
     fp64_nominal = 148 * 128 * 1.965e9 * 1e-12          # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s
+    traffic = profiled_traffic(args.cfg)
     if zg_ms >= loc_ms and zg_ms > 0:
-        ach = zg_flops / (zg_ms * 1e-3) * 1e-12
+        ach = zg_exec / (zg_ms * 1e-3) * 1e-12
+        n_cn, n_nn = stages.get("zgemm_cn", (0.0, 0))[1], stages.get("zgemm_nn", (0.0, 0))[1]
+        t_cn, t_nn = traffic.get("zgemm_cn"), traffic.get("zgemm_nn")
         roofline = {"bound": "tensor", "kernel": "k_zgemm3m_tma (3M complex product on DMMA m8n8k4.f64, TMA-fed; CN + NN instantiations)",
                     "achieved": ach, "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma,
                     "peak_source": "pwh_probe_fp64_tensor_peak, register-resident DMMA loop measured in this run "
-                                   f"(nominal 148 SM x 128 flop/clk x 1.965 GHz = {fp64_nominal:.1f})",
+                                   f"(nominal 148 SM x 128 flop/clk x 1.965 GHz = {fp64_nominal:.1f}); MEASURED_PEAKS.json "
+                                   "holds no FP64 figure",
                     "frac_of_nominal": ach / fp64_nominal,
-                    "flops_per_launch": zg_flops / max(zg_n, 1), "ms_per_launch": zg_ms / max(zg_n, 1),
-                    "pipe_busy_frac": 0.75 * ach / peak_dmma,
-                    "note": "flops counted as 8mnk per complex GEMM (SURVEY.md 8d-4) while the 3M product spends 6mnk on "
-                            "the pipe, so frac can exceed 1; pipe_busy_frac = 0.75 x frac is the share of the DMMA peak "
-                            "actually occupied (ncu pipe_tensor: 90.4 % CN / 85.5 % NN, profiles/r01e_cfg4.md)",
-                    "traffic": PROFILED_TRAFFIC.get(("zgemm", args.cfg))}
+                    "flops_per_launch": zg_exec / max(zg_n, 1), "ms_per_launch": zg_ms / max(zg_n, 1),
+                    "equiv_8mnk_TFLOPs": zg_def / (zg_ms * 1e-3) * 1e-12,
+                    "note": "achieved = flops the kernels execute on the DMMA pipe (3M complex product: 6 m n k; Hermitian "
+                            "Gram: computed tiles only) / event time, so frac <= 1; equiv_8mnk_TFLOPs counts the same "
+                            "launches as 8 m n k per complex GEMM (SURVEY.md 8d-4) for comparison with 4M libraries",
+                    "traffic": ((n_cn * t_cn + n_nn * t_nn) / max(n_cn + n_nn, 1)) if t_cn and t_nn else None,
+                    "traffic_source": traffic.get("source")}
     else:
         ach = loc_bytes / (loc_ms * 1e-3) * 1e-9
-        roofline = {"bound": "hbm", "kernel": "kz_scatter_zinv + kv2_plane + kz_zfwd_gather (local potential + recurrence)",
+        roofline = {"bound": "hbm", "kernel": "local-potential kernels (scatter + z, plane, z + gather + recurrence)",
                     "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "peak_source": hbm_src,
-                    "traffic": PROFILED_TRAFFIC.get(("local", args.cfg))}
-    local_roof = {"ms_per_step": loc_ms / args.steps,
+                    "bytes_per_launch": loc_bytes / max(loc_n, 1), "ms_per_launch": loc_ms / max(loc_n, 1),
+                    "traffic": traffic.get("local"), "traffic_source": traffic.get("source")}
+    local_roof = {"ms_per_step": loc_ms / psteps, "us_per_band_application": 1e3 * loc_ms / max(band_apps, 1),
                   "alg_GBps": loc_bytes / max(loc_ms, 1e-9) * 1e-6, "hbm_frac": loc_bytes / max(loc_ms, 1e-9) * 1e-6 / hbm_peak,
                   "alg_fp64_TFLOPs": loc_flops / max(loc_ms, 1e-9) * 1e-9,
                   "fp64_frac_of_nominal": loc_flops / max(loc_ms, 1e-9) * 1e-9 / fp64_nominal}
-    zgemm_roof = {"ms_per_step": zg_ms / args.steps, "TFLOPs": zg_flops / max(zg_ms, 1e-9) * 1e-9,
-                  "frac_of_probe": zg_flops / max(zg_ms, 1e-9) * 1e-9 / peak_dmma}
+    zgemm_roof = {"ms_per_step": zg_ms / psteps, "executed_TFLOPs": zg_exec / max(zg_ms, 1e-9) * 1e-9,
+                  "pipe_frac_of_probe": zg_exec / max(zg_ms, 1e-9) * 1e-9 / peak_dmma,
+                  "equiv_8mnk_TFLOPs": zg_def / max(zg_ms, 1e-9) * 1e-9}
 
     # ---- end to end through the public host-buffer API: pinned host Psi -> device -> path -> host (every step)
     e2e = None
@@ -396,7 +426,7 @@ def run_ours(args):
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "cpu_baseline": cpu,
             "stages": stage_out, "local_stage": local_roof, "zgemm_stage": zgemm_roof,
-            "ms_per_step_profiled_pass": ms_step_profiled}
+            "ms_per_step_profiled_pass": ms_step_profiled, "profiled_steps": psteps, "kernels": ham.kernels()}
     print(json.dumps(line))
     if dist is not None:
         dist.barrier()
@@ -404,17 +434,31 @@ def run_ours(args):
     return 0
 
 
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full` captures
-# under profiles/ -- filled in per round; None where no capture exists for that config.
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full` captures
-# (profiles/r01e_cfg4.md: CN 6.35 GB, NN 6.82 GB, cold cache; profiles/r01c_cfg3_ncu_full.md for cfg 3), averaged over
-# the CN and NN launches like `achieved`
-PROFILED_TRAFFIC = {("zgemm", 4): 0.5 * (6.231801e9 + 0.120861e9 + 4.602920e9 + 2.220826e9),
-                    ("zgemm", 3): 0.5 * (1.032454e9 + 0.081808e9 + 0.953950e9 + 0.433480e9)}
+def profiled_traffic(cfg: int) -> dict:
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernels, read from the
+    committed summary of the `ncu --set full` captures (profiles/ncu_traffic.json; each entry names the capture it was
+    taken from).  Empty when no capture exists for this config."""
+    try:
+        return dict(json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get(f"cfg{cfg}", {}))
+    except Exception:
+        return {}
+
+
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no launcher: start N ranks (one per GPU) the way the driver does."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -19,6 +19,16 @@
  *     void*; NULL = the legacy default stream) and is asynchronous: results are valid once the caller has
  *     synchronised that stream.  The *_host entry points synchronise before returning.
  *   - One handle may be used from one stream at a time.  There is no CPU fallback of any kind.
+ *   - Several handles may be alive at once (one per k-point is the normal use); they share nothing.
+ *
+ * Environment switches.  They exist for the test-suite, select a KERNEL FAMILY (never a CPU path), are sampled once per
+ * pwh_ham_setup call and never on a launch path:
+ *     PWH_FORCE_GENERIC_FFT=1  generic radix-2/3/4/5/8 shared-memory stage plan instead of the register-resident two-pass
+ *                              transforms (otherwise used only for axis lengths that do not factor as r1 * r2);
+ *     PWH_NO_V2=1              generic-size plane kernel instead of the size-specialised one;
+ *     PWH_NO_ZW=1              CTA-per-column-group z kernels instead of the warp-private ones;
+ *     PWH_ZGEMM_NO_TMA=1       cp.async-fed ZGEMM instead of the TMA-fed one (process-wide, until the next setup).
+ * pwh_ham_kernels() reports which family a handle uses.
  */
 #ifndef PWHAM_H
 #define PWHAM_H
@@ -103,6 +113,16 @@ int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny
              pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream);
 
 /*
+ * pwh_gram_herm -- the same product for a G the caller knows to be Hermitian: G = X^H (A X) with A Hermitian, i.e. the
+ * Rayleigh-Ritz matrices H_Psi = Psi^H (H Psi) and S_Psi = Psi^H Psi of PAPER.md:153-163 (Algorithm 5 steps 1-2).  Only the
+ * tiles on or above the block diagonal are computed on the tensor pipe; the strictly lower blocks are written as the
+ * conjugates of their mirror images (so G[i,j] == conj(G[j,i]) exactly outside the 128 x 128 diagonal blocks and to
+ * rounding inside them).  If X^H Y is not Hermitian the lower blocks are simply not X^H Y.  Workspace as for pwh_gram.
+ */
+int pwh_gram_herm(int64_t npw, int64_t n, const pwh_c128* X, int64_t ldx, const pwh_c128* Y, int64_t ldy, pwh_c128* G,
+                  int64_t ldg, void* ws, size_t ws_bytes, void* stream);
+
+/*
  * Host-buffer entry points (end-to-end path: the paper keeps Psi on the device and moves it host->device once per
  * k-point and SCF step, Algorithm 3).  All pointers below marked HOST are host memory (pinned
  * memory gives asynchronous copies; pageable memory works).  Device staging buffers are allocated on first use,
@@ -157,6 +177,10 @@ int pwh_probe_fp64_tensor_peak(int iters, double* tflops, void* stream);
 
 /* Introspection: fills info[0..7] = {npw, nproj, n1, n2, n3, n_zcolumns, n_xlines, reserved}. */
 int pwh_ham_info(const pwh_ham* ham, int64_t info[8]);
+
+/* Introspection: writes a NUL-terminated, space-separated list of the kernel families this handle launches (e.g.
+ * "kz_scatter_zinv kv2_plane kz_zfwd_gather zgemm3m_tma") into buf (HOST, at most n bytes, truncated). */
+int pwh_ham_kernels(const pwh_ham* ham, char* buf, size_t n);
 
 /* Thread-local message describing the last error returned on this thread ("" if none). */
 const char* pwh_last_error(void);

@@ -21,7 +21,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpwham.so")
 
 EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply_h", "pwh_cheb_filter",
-           "pwh_gram_workspace_bytes", "pwh_gram", "pwh_apply_h_host", "pwh_cheb_filter_host", "pwh_sweep_host",
+           "pwh_gram_workspace_bytes", "pwh_gram", "pwh_gram_herm", "pwh_ham_kernels", "pwh_apply_h_host", "pwh_cheb_filter_host", "pwh_sweep_host",
            "pwh_launch_count", "pwh_ham_info", "pwh_last_error", "pwh_profile_begin", "pwh_profile_end",
            "pwh_probe_fp64_tensor_peak"]
 
@@ -58,6 +58,10 @@ def load_library() -> ctypes.CDLL:
     L.pwh_gram_workspace_bytes.restype = sz
     L.pwh_gram.argtypes = [i64, i64, vp, i64, i64, vp, i64, vp, i64, vp, sz, vp]
     L.pwh_gram.restype = i32
+    L.pwh_gram_herm.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, sz, vp]
+    L.pwh_gram_herm.restype = i32
+    L.pwh_ham_kernels.argtypes = [vp, ctypes.c_char_p, sz]
+    L.pwh_ham_kernels.restype = i32
     L.pwh_apply_h_host.argtypes = [vp, i64, vp, i64, vp, i64, vp]
     L.pwh_apply_h_host.restype = i32
     L.pwh_cheb_filter_host.argtypes = [vp, i64, i64, vp, i64, i32, dbl, dbl, dbl, vp]
@@ -129,6 +133,12 @@ class Ham:
         keys = ["npw", "nproj", "n1", "n2", "n3", "n_zcolumns", "n_xlines", "band_group"]
         return dict(zip(keys, [int(v) for v in arr]))
 
+    def kernels(self) -> list:
+        """pwh_ham_kernels: the kernel families this handle launches."""
+        buf = ctypes.create_string_buffer(256)
+        _check(load_library().pwh_ham_kernels(self.handle, buf, 256), "pwh_ham_kernels")
+        return buf.value.decode().split()
+
     def destroy(self) -> None:
         if self.handle:
             load_library().pwh_ham_destroy(self.handle)
@@ -161,12 +171,16 @@ def ham_setup(lattice, kpt, fft_dims, gvec, vloc, proj, dij, device="cuda:0") ->
     if proj is None or len(proj) == 0:
         nproj, p, d, p_ptr, d_ptr, ldp = 0, None, None, None, None, npw
     else:
-        p = _dev_tensor(proj, torch.complex128, device)
+        if isinstance(proj, torch.Tensor) and proj.is_cuda and proj.dtype == torch.complex128 and proj.dim() == 2 \
+                and proj.stride(1) == 1 and (proj.shape[0] == 1 or proj.stride(0) >= proj.shape[1]):
+            p = proj                                  # borrowed as is: rows may be padded (ldp = stride(0) > npw)
+        else:
+            p = _dev_tensor(proj, torch.complex128, device)
         d = _dev_tensor(dij, torch.float64, device)
         nproj = int(p.shape[0])
         if p.shape[1] != npw or d.shape[0] != nproj:
             raise PwhamError("proj must be (nproj, npw) and dij (nproj,)")
-        p_ptr, d_ptr, ldp = p.data_ptr(), d.data_ptr(), npw
+        p_ptr, d_ptr, ldp = p.data_ptr(), d.data_ptr(), (int(p.stride(0)) if nproj > 1 else max(npw, int(p.stride(0))))
     handle = ctypes.c_void_p()
     with torch.cuda.device(device):
         rc = L.pwh_ham_setup(ctypes.byref(handle), lattice.ctypes.data, kpt.ctypes.data, dims.ctypes.data, npw,
@@ -210,8 +224,9 @@ def cheb_filter(ham: Ham, psi: torch.Tensor, degree: int, a: float, b: float, a0
 _gram_ws = {}
 
 
-def gram(x: torch.Tensor, y: torch.Tensor) -> torch.Tensor:
-    """pwh_gram: returns G of shape (nx, ny) with G[i, j] = <x_i, y_j> = sum_g conj(x[i, g]) y[j, g]."""
+def gram(x: torch.Tensor, y: torch.Tensor, hermitian: bool = False) -> torch.Tensor:
+    """pwh_gram (pwh_gram_herm when `hermitian`): returns G of shape (nx, ny) with G[i, j] = <x_i, y_j> =
+    sum_g conj(x[i, g]) y[j, g]."""
     L = load_library()
     npw = int(x.shape[1])
     x_ptr, ldx = _block_args(x, npw, "x")
@@ -225,9 +240,15 @@ def gram(x: torch.Tensor, y: torch.Tensor) -> torch.Tensor:
         _gram_ws[key] = None
         ws = _gram_ws[key] = torch.empty(need, dtype=torch.uint8, device=x.device)
     with torch.cuda.device(x.device):
-        rc = L.pwh_gram(npw, nx, x_ptr, ldx, ny, y_ptr, ldy, g_cm.data_ptr(), nx, ws.data_ptr(), ws.numel(),
-                        _stream_ptr(x.device))
-    _check(rc, "pwh_gram")
+        if hermitian:
+            if nx != ny:
+                raise PwhamError("hermitian gram needs nx == ny")
+            rc = L.pwh_gram_herm(npw, nx, x_ptr, ldx, y_ptr, ldy, g_cm.data_ptr(), nx, ws.data_ptr(), ws.numel(),
+                                 _stream_ptr(x.device))
+        else:
+            rc = L.pwh_gram(npw, nx, x_ptr, ldx, ny, y_ptr, ldy, g_cm.data_ptr(), nx, ws.data_ptr(), ws.numel(),
+                            _stream_ptr(x.device))
+    _check(rc, "pwh_gram_herm" if hermitian else "pwh_gram")
     return g_cm.T
 
 

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpwham.so")
 SOURCES = ["pwham.cu", "local_kernels.cu", "local_fast.cu", "local_v2.cu", "local_z.cu", "zgemm.cu"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--use_fast_math=false",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-shared"]
 
 
@@ -29,15 +29,30 @@ def needs_build() -> bool:
 
 
 def build_lib(force: bool = False, verbose: bool = False) -> str:
+    """One `nvcc -c` per translation unit (in parallel), then one link step.  Objects go to build/ (git-ignored)."""
     if not force and not needs_build():
         return LIB
-    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
-    cmd = [_nvcc()] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
+    from concurrent.futures import ThreadPoolExecutor
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    cflags = [f for f in NVCC_FLAGS if f != "-shared"] + (["-Xptxas", "-v"] if verbose else [])
+
+    def compile_one(src: str):
+        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        res = subprocess.run([_nvcc()] + cflags + ["-c", "-o", obj, os.path.join(CSRC, src)], capture_output=True, text=True)
+        return src, obj, res
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as ex:
+        results = list(ex.map(compile_one, SOURCES))
+    for src, _, res in results:
+        if verbose or res.returncode != 0:
+            sys.stderr.write(f"--- {src}\n" + res.stdout + res.stderr)
+    if any(res.returncode != 0 for _, _, res in results):
         raise RuntimeError("nvcc failed building libpwham.so")
+    link = subprocess.run([_nvcc(), "-shared", "-o", LIB] + [obj for _, obj, _ in results], capture_output=True, text=True)
+    if link.returncode != 0:
+        sys.stderr.write(link.stdout + link.stderr)
+        raise RuntimeError("nvcc failed linking libpwham.so")
     return LIB
 
 

@@ -54,16 +54,32 @@ void launch_zw_zfwd_gather(const ZPlan& P, const c128* colbuf, const c128* y, in
 
 // zgemm.cu
 cudaError_t zgemm_init();
+// tests only: PWH_ZGEMM_NO_TMA=1, sampled by pwh_ham_setup, routes every ZGEMM through the cp.async kernels
+void zgemm_set_no_tma(bool off);
+// the two TMA descriptors of a handle's projector matrix (opaque 128-byte CUtensorMap images), encoded once at setup
+struct ProjMaps {
+  alignas(64) unsigned char cn[128];
+  alignas(64) unsigned char nn[128];
+  bool ok = false;
+};
+void zgemm_make_proj_maps(ProjMaps& pm, const c128* P, int64_t npw, int64_t nproj, int64_t ldp);
 // runs `ctas` CTAs x 8 warps x iters x 32 DMMA.8x8x4 (512 flop each) and returns the elapsed milliseconds
 cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float* ms);
-// number of K splits chosen for C(M x N) = A^H B with K = npw
-int zgemm_cn_splits(int64_t M, int64_t N, int64_t K);
-size_t zgemm_cn_workspace(int64_t M, int64_t N, int64_t K);
-// C[m + n*ldc] = scale[m] * sum_k conj(A[k + m*lda]) * B[k + n*ldb]      (scale may be null)
+// number of K splits chosen for C(M x N) = A^H B with K = npw (herm: only the block upper triangle is computed)
+int zgemm_cn_splits(int64_t M, int64_t N, int64_t K, bool herm);
+size_t zgemm_cn_workspace(int64_t M, int64_t N, int64_t K, bool herm);
+size_t zgemm_cn_workspace_upto(int64_t M, int64_t N, int64_t K);   // max over n <= N (non-Hermitian)
+// C[m + n*ldc] = scale[m] * sum_k conj(A[k + m*lda]) * B[k + n*ldb]      (scale may be null; pmA: cached maps of A = P;
+// herm: the caller asserts C is Hermitian (M == N), half of the tiles are computed and mirrored)
 void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda, const c128* B, int64_t ldb,
-                     const double* scale, c128* C, int64_t ldc, void* ws, cudaStream_t st);
-// C[m + n*ldc] += alpha * sum_k A[m + k*lda] * B[k + n*ldb]
-void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c128* A, int64_t lda, const c128* B,
-                         int64_t ldb, c128* C, int64_t ldc, cudaStream_t st);
+                     const double* scale, c128* C, int64_t ldc, void* ws, cudaStream_t st, const ProjMaps* pmA = nullptr,
+                     bool herm = false);
+// C[m + n*ldc] = alpha * sum_k A[m + k*lda] * B[k + n*ldb]  (+ C[m + n*ldc] when accumulate)
+void launch_zgemm_nn(int64_t M, int64_t N, int64_t K, double alpha, const c128* A, int64_t lda, const c128* B,
+                     int64_t ldb, c128* C, int64_t ldc, bool accumulate, cudaStream_t st, const ProjMaps* pmA = nullptr);
+
+// pwham.cu: raises the dynamic shared-memory limit of a kernel to the device's opt-in maximum.  The attribute is
+// process-global per kernel, so it is set to the maximum once rather than to one handle's need.
+cudaError_t set_max_dyn_smem(const void* func);
 
 }  // namespace pwh

@@ -52,10 +52,11 @@ __global__ void __launch_bounds__(ZT) k_scatter_zinv(const LocalPlan P, const c1
   }
 }
 
+// `out` may alias `y` or `yprev`: entry g of the three is read and written by the same thread, in that order.
 __global__ void __launch_bounds__(ZT) k_zfwd_gather(const LocalPlan P, const c128* __restrict__ colbuf,
-                                                    const c128* __restrict__ y, int64_t ldy,
-                                                    const c128* __restrict__ yprev, int64_t ldprev,
-                                                    c128* __restrict__ out, int64_t ldout, double alpha, double cshift,
+                                                    const c128* y, int64_t ldy,
+                                                    const c128* yprev, int64_t ldprev,
+                                                    c128* out, int64_t ldout, double alpha, double cshift,
                                                     double beta) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   c128* lines = reinterpret_cast<c128*>(smem_raw);
@@ -152,11 +153,11 @@ size_t plane_smem(const LocalPlan& P) {
 
 cudaError_t local_kernels_init(const LocalPlan& P) {
   cudaError_t e;
-  e = cudaFuncSetAttribute(k_scatter_zinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zkernel_smem(P));
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_scatter_zinv));
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_zfwd_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zkernel_smem(P));
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zfwd_gather));
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_plane, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plane_smem(P));
+  return set_max_dyn_smem(reinterpret_cast<const void*>(&k_plane));
 }
 
 void launch_scatter_zinv(const LocalPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st) {

@@ -20,7 +20,6 @@
 //   * no load or store is predicated: x-lines outside the sphere are read from a zero line and stored to a dump line of
 //     the half-plane, rows outside the disc are read from a zero padding column and stored to a dump padding column
 //     (16 predicates per radix-16 item had to be packed into a register and unpacked again).
-#include <cstdlib>
 #include <type_traits>
 
 #include "fft_reg.cuh"
@@ -259,7 +258,7 @@ __global__ void kv2_perm_vloc(int n1, int n2, int n3, int r1x, int r2x, int r1y,
 
 template <class C>
 cudaError_t v2_init(int nxl) {
-  return cudaFuncSetAttribute(kv2_plane<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes(nxl));
+  return set_max_dyn_smem(reinterpret_cast<const void*>(&kv2_plane<C>));
 }
 template <class C>
 void v2_launch(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st) {
@@ -307,11 +306,6 @@ bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max) {
   else if (n1 == 96) { order[norder++] = 10; order[norder++] = 8; order[norder++] = 2; }
   else if (n1 == 120) { order[norder++] = 5; order[norder++] = 4; }   // 8 warps measured faster than 10 (12.4 vs 12.9 ms, cfg 5)
   else if (n1 == 128) { order[norder++] = 6; order[norder++] = 7; }
-  if (const char* e = getenv("PWH_V2_VARIANT")) {   // measurement aid: force one instantiation
-    const int v = atoi(e);
-    for (int oi = 0; oi < norder; ++oi)
-      if (order[oi] == v) { order[0] = v; norder = 1; break; }
-  }
   for (int oi = 0; oi < norder; ++oi) {
     const int var = order[oi];
     bool ok = false;

@@ -126,10 +126,11 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
   }
 }
 
+// `out` may alias `y` or `yprev`: entry g of the three is read and written by the same thread, in that order.
 __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, const c128* __restrict__ colbuf,
-                                                             const c128* __restrict__ y, int64_t ldy,
-                                                             const c128* __restrict__ yprev, int64_t ldprev,
-                                                             c128* __restrict__ out, int64_t ldout, double alpha,
+                                                             const c128* y, int64_t ldy,
+                                                             const c128* yprev, int64_t ldprev,
+                                                             c128* out, int64_t ldout, double alpha,
                                                              double cshift, double beta, int nb) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   c128* tw = reinterpret_cast<c128*>(smem_raw);
@@ -145,9 +146,9 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
     const int quad = item % P.nq, band = item / P.nq;
     const c128* __restrict__ src = colbuf + (int64_t)band * P.n3 * pstride + quad * cw;
     const int4* __restrict__ tab4 = reinterpret_cast<const int4*>(P.ztab + (int64_t)quad * (r2 * cw * r1p));
-    const c128* __restrict__ yb = y + (int64_t)band * ldy;
-    const c128* __restrict__ pb = (beta != 0.0) ? yprev + (int64_t)band * ldprev : nullptr;
-    c128* __restrict__ ob = out + (int64_t)band * ldout;
+    const c128* yb = y + (int64_t)band * ldy;
+    const c128* pb = (beta != 0.0) ? yprev + (int64_t)band * ldprev : nullptr;
+    c128* ob = out + (int64_t)band * ldout;
     // the epilogue's operands y[g], y_prev[g] come from HBM: start them towards L2 now, the transforms run meanwhile
     for (int i = lane; i < r2 * cw * (r1p / 4); i += 32) {
       const int4 t = __ldg(tab4 + i);
@@ -223,9 +224,9 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
 size_t zw_smem(const ZPlan& P) { return sizeof(c128) * ((size_t)P.n3 + (size_t)ZW * P.cw * P.zs); }
 
 cudaError_t zw_kernels_init(const ZPlan& P) {
-  cudaError_t e = cudaFuncSetAttribute(kz_scatter_zinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zw_smem(P));
+  cudaError_t e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_scatter_zinv));
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(kz_zfwd_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zw_smem(P));
+  return set_max_dyn_smem(reinterpret_cast<const void*>(&kz_zfwd_gather));
 }
 
 static int zw_grid(const ZPlan& P, int nb) {

@@ -15,9 +15,18 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "launch.h"
 
 using namespace pwh;
+
+// NVTX range per stage of the path (the paper isolates its roofline regions the same way);
+// header-only NVTX v3: a no-op unless a profiler injects itself.
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 
 namespace pwh {
 static std::atomic<int64_t> g_launches{0};
@@ -50,6 +59,14 @@ ScopedLaunch::~ScopedLaunch() {
   if (idx_ < 0) return;
   std::lock_guard<std::mutex> lk(g_prof_mu);
   cudaEventRecord(g_prof[(size_t)idx_].e1, st_);
+}
+cudaError_t set_max_dyn_smem(const void* func) {
+  int dev = 0, smem_max = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
 }
 }  // namespace pwh
 
@@ -85,6 +102,7 @@ struct pwh_ham {
   bool zw = false;
   const c128* proj = nullptr;
   int64_t ldp = 0;
+  ProjMaps pmaps;
   double* dij = nullptr;
   int band_group = 1;
   std::vector<void*> allocs;
@@ -219,6 +237,12 @@ static int upload(pwh_ham* h, const std::vector<T>& v, const T** out, cudaStream
   return PWH_OK;
 }
 
+// Kernel-family switches for the tests (documented in include/pwham.h); sampled by pwh_ham_setup only, never on a launch path.
+static bool env_on(const char* name) {
+  const char* e = getenv(name);
+  return e && e[0] == '1';
+}
+
 static int wrapi(int v, int n) {
   int r = v % n;
   return r < 0 ? r + n : r;
@@ -256,11 +280,11 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   FastPlan& fp = h->fp;
   memset(&fp, 0, sizeof(fp));
   {
-    const char* force = getenv("PWH_FORCE_GENERIC_FFT");
-    bool ok = !(force && force[0] == '1');
+    bool ok = !env_on("PWH_FORCE_GENERIC_FFT");
     for (int ax = 0; ax < 3 && ok; ++ax) ok = factor_two_pass(dims[ax], fp.r1[ax], fp.r2[ax]);
     h->fast = ok;
   }
+  zgemm_set_no_tma(env_on("PWH_ZGEMM_NO_TMA"));
   std::vector<c128> tw[3];
   std::vector<int> nat[3];
   for (int ax = 0; ax < 3; ++ax)
@@ -434,10 +458,9 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   // size-specialised plane kernel (local_v2.cu): needs the register-resident z kernels, a box side it is instantiated
   // for, x-lines contiguous modulo n1 and every y-row of the disc a contiguous run of x-lines
   if (h->fast) {
-    const char* off = getenv("PWH_NO_V2");
     V2Plan& vp = h->vp;
     memset(&vp, 0, sizeof(vp));
-    bool ok = !(off && off[0] == '1') && nxl < 65536 && ncols < (1 << 30);
+    bool ok = !env_on("PWH_NO_V2") && nxl < 65536 && ncols < (1 << 30);
     for (int i = 0; i < nxl && ok; ++i) ok = x_of_xl[i] == (x_of_xl[0] + i) % n1;
     std::vector<int2> yrow((size_t)n2, make_int2(0, 0));
     if (ok) {
@@ -485,7 +508,6 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   }
   // warp-private z kernels (local_z.cu): table of plane-wave indices in the order their lanes read it
   if (h->fast) {
-    const char* off = getenv("PWH_NO_ZW");
     ZPlan& zp = h->zp;
     memset(&zp, 0, sizeof(zp));
     zp.n3 = n3; zp.r1 = fp.r1[2]; zp.r2 = fp.r2[2];
@@ -501,7 +523,7 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     zp.zs = zs;
     zp.tw = fp.tw[2];
     zp.kin = lp.kin;
-    if (!(off && off[0] == '1') && zw_smem(zp) <= (size_t)smem_max) {
+    if (!env_on("PWH_NO_ZW") && zw_smem(zp) <= (size_t)smem_max) {
       std::vector<int> ztab((size_t)zp.nq * zp.r2 * zp.cw * zp.r1p, -1);
       for (int64_t i = 0; i < npw; ++i) {
         const int xw = wrapi(g[3 * i], n1), yw = wrapi(g[3 * i + 1], n2), zw_ = wrapi(g[3 * i + 2], n3);
@@ -552,6 +574,7 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   }
 
   CUDA_TRY(zgemm_init());
+  if (nproj > 0) zgemm_make_proj_maps(h->pmaps, h->proj, npw, nproj, ldp);
 
   // bands per launch of the local kernels: the column buffer of a group (written by one kernel, read by the next) should
   // stay in the 126 MB L2 -- at most 56 MB -- and the plane kernel's grid of n3 x bands CTAs (one per SM) should fill
@@ -605,6 +628,21 @@ extern "C" int pwh_ham_info(const pwh_ham* h, int64_t info[8]) {
   return PWH_OK;
 }
 
+extern "C" int pwh_ham_kernels(const pwh_ham* h, char* buf, size_t n) {
+  if (!h || !buf || n == 0) return fail(PWH_EINVAL, "null argument");
+  std::string s;
+  if (h->fast) {
+    s += h->zw ? "kz_scatter_zinv " : "kf_scatter_zinv ";
+    s += h->v2 ? "kv2_plane " : "kf_plane ";
+    s += h->zw ? "kz_zfwd_gather " : "kf_zfwd_gather ";
+  } else {
+    s += "k_scatter_zinv k_plane k_zfwd_gather ";
+  }
+  if (h->nproj > 0) s += h->pmaps.ok ? "zgemm3m_tma" : "zgemm3m";
+  snprintf(buf, n, "%s", s.c_str());
+  return PWH_OK;
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // workspace
 // ---------------------------------------------------------------------------------------------------------------
@@ -614,6 +652,9 @@ struct WsLayout {
   int group;
 };
 
+// Every term is non-decreasing in nband (the split-K scratch is sized for the worst narrower block, because the split
+// count is not monotone in the number of tiles), so a workspace of pwh_workspace_bytes(ham, nband_max) serves every call
+// with nband <= nband_max, as include/pwham.h promises.
 static WsLayout ws_layout(const pwh_ham* h, int64_t nband) {
   WsLayout w;
   w.group = (int)std::min<int64_t>(h->band_group, std::max<int64_t>(nband, 1));
@@ -621,7 +662,7 @@ static WsLayout ws_layout(const pwh_ham* h, int64_t nband) {
   size_t off = 0;
   w.colbuf = off; off += align_up((size_t)w.group * h->n3 * h->lp.ncols_pad * sizeof(c128), 256);
   w.cmat = off;   off += align_up((size_t)std::max<int64_t>(h->nproj, 1) * nband * sizeof(c128), 256);
-  w.part = off;   off += align_up(h->nproj > 0 ? zgemm_cn_workspace(h->nproj, nband, h->npw) : 16, 256);
+  w.part = off;   off += align_up(h->nproj > 0 ? zgemm_cn_workspace_upto(h->nproj, nband, h->npw) : 16, 256);
   w.y1 = off;     off += align_up((size_t)w.ldw * nband * sizeof(c128), 256);
   w.y2 = off;     off += align_up((size_t)w.ldw * nband * sizeof(c128), 256);
   w.total = off;
@@ -633,36 +674,45 @@ extern "C" size_t pwh_workspace_bytes(const pwh_ham* h, int64_t nband_max) {
   return ws_layout(h, std::max<int64_t>(nband_max, 1)).total;
 }
 
-// out = alpha * ((H - c) y) - beta * yprev   for nband bands
+// out = alpha * ((H - c) y) - beta * yprev   for nband bands.  `out` may be the buffer of `yprev` (three-term recurrence
+// in place over Y_{j-1}) or, when yprev is null, the buffer of `y` itself: every kernel that writes out[g] has read y[g]
+// and yprev[g] in the same thread before, and the projector coefficients P^H y are complete before the first write.
 static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c128* yprev, int64_t ldprev, c128* out,
                   int64_t ldout, double alpha, double cshift, double beta, unsigned char* ws, const WsLayout& w,
                   cudaStream_t st) {
   c128* colbuf = reinterpret_cast<c128*>(ws + w.colbuf);
   c128* cmat = reinterpret_cast<c128*>(ws + w.cmat);
-  if (h->nproj > 0)
-    launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, y, ldy, h->dij, cmat, h->nproj, ws + w.part, st);
-  for (int64_t b0 = 0; b0 < nband; b0 += w.group) {
-    const int nb = (int)std::min<int64_t>(w.group, nband - b0);
-    if (h->fast) {
-      if (h->zw) launch_zw_scatter_zinv(h->zp, y + b0 * ldy, ldy, colbuf, nb, st);
-      else launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, colbuf, nb, st);
-      if (h->v2) launch_v2_plane(h->vp, colbuf, nb, st);
-      else launch_fast_plane(h->fp, colbuf, nb, st);
-      if (h->zw)
-        launch_zw_zfwd_gather(h->zp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
-                              out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
-      else
-        launch_fast_zfwd_gather(h->fp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+  if (h->nproj > 0) {
+    NvtxRange r("pwh:nonlocal:C=D.P^H.Y");
+    launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, y, ldy, h->dij, cmat, h->nproj, ws + w.part, st, &h->pmaps);
+  }
+  {
+    NvtxRange r("pwh:local+kinetic+recurrence");
+    for (int64_t b0 = 0; b0 < nband; b0 += w.group) {
+      const int nb = (int)std::min<int64_t>(w.group, nband - b0);
+      if (h->fast) {
+        if (h->zw) launch_zw_scatter_zinv(h->zp, y + b0 * ldy, ldy, colbuf, nb, st);
+        else launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, colbuf, nb, st);
+        if (h->v2) launch_v2_plane(h->vp, colbuf, nb, st);
+        else launch_fast_plane(h->fp, colbuf, nb, st);
+        if (h->zw)
+          launch_zw_zfwd_gather(h->zp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
                                 out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
-    } else {
-      launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, colbuf, nb, st);
-      launch_plane(h->lp, colbuf, nb, st);
-      launch_zfwd_gather(h->lp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
-                         out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+        else
+          launch_fast_zfwd_gather(h->fp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                                  out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+      } else {
+        launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, colbuf, nb, st);
+        launch_plane(h->lp, colbuf, nb, st);
+        launch_zfwd_gather(h->lp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                           out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+      }
     }
   }
-  if (h->nproj > 0)
-    launch_zgemm_nn_acc(h->npw, nband, h->nproj, alpha, h->proj, h->ldp, cmat, h->nproj, out, ldout, st);
+  if (h->nproj > 0) {
+    NvtxRange r("pwh:nonlocal:Y+=a.P.C");
+    launch_zgemm_nn(h->npw, nband, h->nproj, alpha, h->proj, h->ldp, cmat, h->nproj, out, ldout, true, st, &h->pmaps);
+  }
   CUDA_TRY(cudaGetLastError());
   return PWH_OK;
 }
@@ -675,6 +725,13 @@ static int check_ws(const pwh_ham* h, int64_t nband, void* ws, size_t ws_bytes) 
   return PWH_OK;
 }
 
+// do the address ranges of two column-major blocks (npw x nband, leading dimensions lda / ldb) intersect?
+static bool blocks_overlap(const void* a, int64_t lda, const void* b, int64_t ldb, int64_t npw, int64_t nband) {
+  const uintptr_t a0 = (uintptr_t)a, a1 = a0 + ((size_t)(nband - 1) * lda + npw) * sizeof(c128);
+  const uintptr_t b0 = (uintptr_t)b, b1 = b0 + ((size_t)(nband - 1) * ldb + npw) * sizeof(c128);
+  return a0 < b1 && b0 < a1;
+}
+
 extern "C" int pwh_apply_h(pwh_ham* h, int64_t nband, const pwh_c128* psi, int64_t ldpsi, pwh_c128* hpsi, int64_t ldh,
                            void* ws, size_t ws_bytes, void* stream) {
   if (!h) return fail(PWH_EINVAL, "handle is null");
@@ -684,6 +741,8 @@ extern "C" int pwh_apply_h(pwh_ham* h, int64_t nband, const pwh_c128* psi, int64
   if (ldpsi < h->npw || ldh < h->npw) return fail(PWH_EINVAL, "leading dimension smaller than npw");
   int rc = check_ws(h, nband, ws, ws_bytes);
   if (rc) return rc;
+  if (blocks_overlap(psi, ldpsi, hpsi, ldh, h->npw, nband)) return fail(PWH_EINVAL, "psi and hpsi overlap");
+  NvtxRange r("pwh_apply_h");
   const WsLayout w = ws_layout(h, nband);
   return h_step(h, nband, reinterpret_cast<const c128*>(psi), ldpsi, nullptr, 0, reinterpret_cast<c128*>(hpsi), ldh, 1.0,
                 0.0, 0.0, reinterpret_cast<unsigned char*>(ws), w, (cudaStream_t)stream);
@@ -701,39 +760,51 @@ extern "C" int pwh_cheb_filter(pwh_ham* h, int64_t nband, pwh_c128* psi, int64_t
   if (ld < h->npw) return fail(PWH_EINVAL, "ld < npw");
   int rc = check_ws(h, nband, ws, ws_bytes);
   if (rc) return rc;
+  NvtxRange r("pwh_cheb_filter");
   const WsLayout w = ws_layout(h, nband);
   unsigned char* wsb = reinterpret_cast<unsigned char*>(ws);
   cudaStream_t st = (cudaStream_t)stream;
   c128* buf[3] = {reinterpret_cast<c128*>(psi), reinterpret_cast<c128*>(wsb + w.y1), reinterpret_cast<c128*>(wsb + w.y2)};
   const int64_t lds[3] = {ld, w.ldw, w.ldw};
   const double e = 0.5 * (b - a), c = 0.5 * (b + a), sigma1 = e / (a0 - c);
+  // Where Y_j lives (0 = psi, 1 and 2 = workspace), chosen so that Y_degree lands in psi without a final copy:
+  // from the second (even degree) or fourth (odd degree) step on, Y_{j+1} is written over Y_{j-1}, which the
+  // recurrence reads for the last time in that very step; Y_1 of a degree-1 filter is written over Y_0 itself.
+  std::vector<int> where((size_t)degree + 1, 0);
+  if (degree % 2 == 0) {
+    where[1] = 1;
+    for (int j = 2; j <= degree; ++j) where[j] = where[j - 2];
+  } else if (degree >= 3) {
+    where[1] = 1; where[2] = 2; where[3] = 0;
+    for (int j = 4; j <= degree; ++j) where[j] = where[j - 2];
+  }
   double sigma = sigma1;
   // Y_1 = (sigma_1/e) (H - c) Y_0
-  rc = h_step(h, nband, buf[0], lds[0], nullptr, 0, buf[1], lds[1], sigma1 / e, c, 0.0, wsb, w, st);
+  rc = h_step(h, nband, buf[0], lds[0], nullptr, 0, buf[where[1]], lds[where[1]], sigma1 / e, c, 0.0, wsb, w, st);
   if (rc) return rc;
   for (int j = 1; j < degree; ++j) {
     const double sigma_new = 1.0 / (2.0 / sigma1 - sigma);
-    const int ip = (j - 1) % 3, ic = j % 3, io = (j + 1) % 3;
+    const int ip = where[j - 1], ic = where[j], io = where[j + 1];
     rc = h_step(h, nband, buf[ic], lds[ic], buf[ip], lds[ip], buf[io], lds[io], 2.0 * sigma_new / e, c,
                 sigma * sigma_new, wsb, w, st);
     if (rc) return rc;
     sigma = sigma_new;
   }
-  const int fin = degree % 3;
-  if (fin != 0)
-    CUDA_TRY(cudaMemcpy2DAsync(psi, (size_t)ld * sizeof(c128), buf[fin], (size_t)lds[fin] * sizeof(c128),
-                               (size_t)h->npw * sizeof(c128), (size_t)nband, cudaMemcpyDeviceToDevice, st));
   return PWH_OK;
 }
 
 extern "C" size_t pwh_gram_workspace_bytes(int64_t npw, int64_t nx, int64_t ny) {
   if (npw < 1 || nx < 1 || ny < 1) return 256;
-  return align_up(zgemm_cn_workspace(nx, ny, npw), 256);
+  // the Hermitian variant computes fewer tiles and may choose more K splits: size for both
+  size_t need = zgemm_cn_workspace(nx, ny, npw, false);
+  if (nx == ny) need = std::max(need, zgemm_cn_workspace(nx, ny, npw, true));
+  return align_up(need, 256);
 }
 
-extern "C" int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny, const pwh_c128* Y,
-                        int64_t ldy, pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream) {
+static int gram_impl(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny, const pwh_c128* Y, int64_t ldy,
+                     pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream, bool herm) {
   if (npw < 1 || nx < 0 || ny < 0) return fail(PWH_EINVAL, "bad sizes");
+  if (herm && nx != ny) return fail(PWH_EINVAL, "a Hermitian Gram matrix needs nx == ny");
   if (nx == 0 || ny == 0) return PWH_OK;
   if (nx > INT32_MAX / 2 || ny > INT32_MAX / 2) return fail(PWH_EINVAL, "nx / ny too large");
   if (!X || !Y || !G) return fail(PWH_EINVAL, "null argument");
@@ -741,10 +812,21 @@ extern "C" int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx,
   if (!ws || (uintptr_t)ws % 256 != 0) return fail(PWH_EINVAL, "workspace null or not 256-byte aligned");
   if (ws_bytes < pwh_gram_workspace_bytes(npw, nx, ny)) return fail(PWH_EINVAL, "workspace too small");
   CUDA_TRY(zgemm_init());
+  NvtxRange r(herm ? "pwh_gram_herm" : "pwh_gram");
   launch_zgemm_cn(nx, ny, npw, reinterpret_cast<const c128*>(X), ldx, reinterpret_cast<const c128*>(Y), ldy, nullptr,
-                  reinterpret_cast<c128*>(G), ldg, ws, (cudaStream_t)stream);
+                  reinterpret_cast<c128*>(G), ldg, ws, (cudaStream_t)stream, nullptr, herm);
   CUDA_TRY(cudaGetLastError());
   return PWH_OK;
+}
+
+extern "C" int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny, const pwh_c128* Y,
+                        int64_t ldy, pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream) {
+  return gram_impl(npw, nx, X, ldx, ny, Y, ldy, G, ldg, ws, ws_bytes, stream, false);
+}
+
+extern "C" int pwh_gram_herm(int64_t npw, int64_t n, const pwh_c128* X, int64_t ldx, const pwh_c128* Y, int64_t ldy,
+                             pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream) {
+  return gram_impl(npw, n, X, ldx, n, Y, ldy, G, ldg, ws, ws_bytes, stream, true);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -760,14 +842,20 @@ static int ensure(void** p, size_t* have, size_t need) {
   return PWH_OK;
 }
 
-extern "C" int pwh_apply_h_host(pwh_ham* h, int64_t nband, const pwh_c128* psi_host, int64_t ldpsi, pwh_c128* hpsi_host,
-                                int64_t ldh, void* stream) {
-  if (!h) return fail(PWH_EINVAL, "handle is null");
-  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
-  if (nband == 0) return PWH_OK;
-  if (!psi_host || !hpsi_host) return fail(PWH_EINVAL, "null argument");
-  if (ldpsi < h->npw || ldh < h->npw) return fail(PWH_EINVAL, "leading dimension smaller than npw");
-  cudaStream_t st = (cudaStream_t)stream;
+// Every exit of a host entry point -- success or error -- waits for the caller's stream and the two copy streams, so no
+// copy into or out of the caller's host buffers is still in flight when the call returns (include/pwham.h).
+static int host_finish(pwh_ham* h, cudaStream_t st, int rc) {
+  const cudaError_t e0 = cudaStreamSynchronize(st);
+  const cudaError_t e1 = h->cs_in ? cudaStreamSynchronize(h->cs_in) : cudaSuccess;
+  const cudaError_t e2 = h->cs_out ? cudaStreamSynchronize(h->cs_out) : cudaSuccess;
+  if (rc != PWH_OK) return rc;
+  for (cudaError_t e : {e0, e1, e2})
+    if (e != cudaSuccess) return fail(PWH_ECUDA, "stream synchronisation: %s", cudaGetErrorString(e));
+  return PWH_OK;
+}
+
+static int apply_h_host_impl(pwh_ham* h, int64_t nband, const pwh_c128* psi_host, int64_t ldpsi, pwh_c128* hpsi_host,
+                             int64_t ldh, cudaStream_t st) {
   const size_t blk = (size_t)h->npw * nband * sizeof(c128), row = (size_t)h->npw * sizeof(c128);
   int rc;
   if ((rc = ensure(&h->st_psi, &h->st_psi_bytes, blk))) return rc;
@@ -777,8 +865,18 @@ extern "C" int pwh_apply_h_host(pwh_ham* h, int64_t nband, const pwh_c128* psi_h
   rc = pwh_apply_h(h, nband, (const pwh_c128*)h->st_psi, h->npw, (pwh_c128*)h->st_hpsi, h->npw, h->st_ws, h->st_ws_bytes, st);
   if (rc) return rc;
   CUDA_TRY(cudaMemcpy2DAsync(hpsi_host, (size_t)ldh * sizeof(c128), h->st_hpsi, row, row, nband, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(cudaStreamSynchronize(st));
   return PWH_OK;
+}
+
+extern "C" int pwh_apply_h_host(pwh_ham* h, int64_t nband, const pwh_c128* psi_host, int64_t ldpsi, pwh_c128* hpsi_host,
+                                int64_t ldh, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (nband == 0) return PWH_OK;
+  if (!psi_host || !hpsi_host) return fail(PWH_EINVAL, "null argument");
+  if (ldpsi < h->npw || ldh < h->npw) return fail(PWH_EINVAL, "leading dimension smaller than npw");
+  cudaStream_t st = (cudaStream_t)stream;
+  return host_finish(h, st, apply_h_host_impl(h, nband, psi_host, ldpsi, hpsi_host, ldh, st));
 }
 
 static int filter_blocks(pwh_ham* h, int64_t nband, int64_t block, c128* psi_dev, int64_t ld, int degree, double a,
@@ -842,6 +940,15 @@ static int filter_pipelined(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* 
   return PWH_OK;
 }
 
+static int cheb_filter_host_impl(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
+                                 double a, double b, double a0, cudaStream_t st) {
+  const size_t blk = (size_t)h->npw * nband * sizeof(c128);
+  int rc;
+  if ((rc = ensure(&h->st_psi, &h->st_psi_bytes, blk))) return rc;
+  if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, pwh_workspace_bytes(h, std::min(block, pipeline_chunk(nband, block)))))) return rc;
+  return filter_pipelined(h, nband, block, psi_host, ld, degree, a, b, a0, st);
+}
+
 extern "C" int pwh_cheb_filter_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
                                     double a, double b, double a0, void* stream) {
   if (!h) return fail(PWH_EINVAL, "handle is null");
@@ -852,27 +959,12 @@ extern "C" int pwh_cheb_filter_host(pwh_ham* h, int64_t nband, int64_t block, pw
   if (ld < h->npw) return fail(PWH_EINVAL, "ld < npw");
   cudaStream_t st = (cudaStream_t)stream;
   if (block <= 0 || block > nband) block = nband;
-  const size_t blk = (size_t)h->npw * nband * sizeof(c128);
-  int rc;
-  if ((rc = ensure(&h->st_psi, &h->st_psi_bytes, blk))) return rc;
-  if ((rc = ensure(&h->st_ws, &h->st_ws_bytes, pwh_workspace_bytes(h, std::min(block, pipeline_chunk(nband, block)))))) return rc;
-  if ((rc = filter_pipelined(h, nband, block, psi_host, ld, degree, a, b, a0, st))) return rc;
-  CUDA_TRY(cudaStreamSynchronize(st));
-  CUDA_TRY(cudaStreamSynchronize(h->cs_out));
-  return PWH_OK;
+  return host_finish(h, st, cheb_filter_host_impl(h, nband, block, psi_host, ld, degree, a, b, a0, st));
 }
 
-extern "C" int pwh_sweep_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
-                              double a, double b, double a0, pwh_c128* hpsi_host, int64_t ldh, pwh_c128* G_host,
-                              int64_t ldg, void* stream) {
-  if (!h) return fail(PWH_EINVAL, "handle is null");
-  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
-  if (degree < 0 || !(b > a) || !(a0 < a)) return fail(PWH_EINVAL, "bad filter parameters");
-  if (nband == 0) return PWH_OK;
-  if (!psi_host || !G_host) return fail(PWH_EINVAL, "null argument");
-  if (ld < h->npw || ldg < nband || (hpsi_host && ldh < h->npw)) return fail(PWH_EINVAL, "leading dimension too small");
-  cudaStream_t st = (cudaStream_t)stream;
-  if (block <= 0 || block > nband) block = nband;
+static int sweep_host_impl(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree, double a,
+                           double b, double a0, pwh_c128* hpsi_host, int64_t ldh, pwh_c128* G_host, int64_t ldg,
+                           cudaStream_t st) {
   const size_t blk = (size_t)h->npw * nband * sizeof(c128), row = (size_t)h->npw * sizeof(c128);
   const size_t gbytes = (size_t)nband * nband * sizeof(c128);
   const size_t wsb = std::max(pwh_workspace_bytes(h, block), pwh_gram_workspace_bytes(h->npw, nband, nband));
@@ -888,16 +980,29 @@ extern "C" int pwh_sweep_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128
                      (pwh_c128*)((c128*)h->st_hpsi + b0 * h->npw), h->npw, h->st_ws, h->st_ws_bytes, st);
     if (rc) return rc;
   }
-  rc = pwh_gram(h->npw, nband, (const pwh_c128*)h->st_psi, h->npw, nband, (const pwh_c128*)h->st_hpsi, h->npw,
-                (pwh_c128*)h->st_g, nband, h->st_ws, h->st_ws_bytes, st);
+  // Psi^H (H Psi) is Hermitian: half of its tiles are computed, the rest mirrored
+  rc = pwh_gram_herm(h->npw, nband, (const pwh_c128*)h->st_psi, h->npw, (const pwh_c128*)h->st_hpsi, h->npw,
+                     (pwh_c128*)h->st_g, nband, h->st_ws, h->st_ws_bytes, st);
   if (rc) return rc;
   if (hpsi_host)
     CUDA_TRY(cudaMemcpy2DAsync(hpsi_host, (size_t)ldh * sizeof(c128), h->st_hpsi, row, row, nband, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaMemcpy2DAsync(G_host, (size_t)ldg * sizeof(c128), h->st_g, (size_t)nband * sizeof(c128),
                              (size_t)nband * sizeof(c128), nband, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(cudaStreamSynchronize(st));
-  CUDA_TRY(cudaStreamSynchronize(h->cs_out));
   return PWH_OK;
+}
+
+extern "C" int pwh_sweep_host(pwh_ham* h, int64_t nband, int64_t block, pwh_c128* psi_host, int64_t ld, int degree,
+                              double a, double b, double a0, pwh_c128* hpsi_host, int64_t ldh, pwh_c128* G_host,
+                              int64_t ldg, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (degree < 0 || !(b > a) || !(a0 < a)) return fail(PWH_EINVAL, "bad filter parameters");
+  if (nband == 0) return PWH_OK;
+  if (!psi_host || !G_host) return fail(PWH_EINVAL, "null argument");
+  if (ld < h->npw || ldg < nband || (hpsi_host && ldh < h->npw)) return fail(PWH_EINVAL, "leading dimension too small");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (block <= 0 || block > nband) block = nband;
+  return host_finish(h, st, sweep_host_impl(h, nband, block, psi_host, ld, degree, a, b, a0, hpsi_host, ldh, G_host, ldg, st));
 }
 
 extern "C" int pwh_probe_fp64_tensor_peak(int iters, double* tflops, void* stream) {
@@ -924,17 +1029,25 @@ extern "C" int pwh_profile_begin(void) {
 extern "C" int pwh_profile_end(double ms[PWH_NSTAGES], int64_t launches[PWH_NSTAGES]) {
   if (!ms || !launches) return fail(PWH_EINVAL, "null argument");
   g_prof_on.store(false);
-  CUDA_TRY(cudaDeviceSynchronize());
+  const cudaError_t esync = cudaDeviceSynchronize();
   std::lock_guard<std::mutex> lk(g_prof_mu);
+  if (esync != cudaSuccess) {
+    for (auto& r : g_prof) { g_prof_pool.push_back(r.e0); g_prof_pool.push_back(r.e1); }
+    g_prof.clear();
+    return fail(PWH_ECUDA, "cudaDeviceSynchronize: %s", cudaGetErrorString(esync));
+  }
   for (int i = 0; i < PWH_NSTAGES; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  cudaError_t first = cudaSuccess;
   for (auto& r : g_prof) {
     float t = 0.f;
-    CUDA_TRY(cudaEventElapsedTime(&t, r.e0, r.e1));
-    if (r.stage >= 0 && r.stage < PWH_NSTAGES) { ms[r.stage] += (double)t; launches[r.stage] += 1; }
+    const cudaError_t e = cudaEventElapsedTime(&t, r.e0, r.e1);
+    if (e != cudaSuccess && first == cudaSuccess) first = e;
+    if (e == cudaSuccess && r.stage >= 0 && r.stage < PWH_NSTAGES) { ms[r.stage] += (double)t; launches[r.stage] += 1; }
     g_prof_pool.push_back(r.e0);
     g_prof_pool.push_back(r.e1);
   }
   g_prof.clear();
+  if (first != cudaSuccess) return fail(PWH_ECUDA, "cudaEventElapsedTime: %s", cudaGetErrorString(first));
   return PWH_OK;
 }
 

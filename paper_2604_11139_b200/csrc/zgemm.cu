@@ -4,15 +4,17 @@
 //                                        Rayleigh-Ritz Gram product Psi^H (H Psi), split over K
 //   "NN":  C += alpha A B with K = nproj -> P . (D . P^H psi) accumulated onto the recurrence term
 // tcgen05 has no f64 kind, so FP64 contractions on sm_100a are warp-level DMMA with register accumulators
-// (measured on B200: DMMA.8x8x4 peak 37.1 TFLOP/s == DFMA peak).  Three generations of the kernel live here:
+// (measured on B200: DMMA.8x8x4 peak 37.1 TFLOP/s == DFMA peak).  Two kernels live here:
 //   k_zgemm3m_tma  (default)  3M complex product, operand slabs by TMA with 128-byte swizzle, mbarrier hand-over
-//   k_zgemm3m      (fallback) 3M, slabs by cp.async into padded layouts, same mbarrier hand-over  (PWH_ZGEMM_NO_TMA=1)
-//   k_zgemm        (reference) four real DMMAs per complex product, cp.async + __syncthreads     (PWH_ZGEMM_4M=1)
+//   k_zgemm3m      (fallback) 3M, slabs by cp.async into padded layouts, same mbarrier hand-over; used when the driver
+//                             does not export cuTensorMapEncodeTiled or refuses an operand (PWH_ZGEMM_NO_TMA=1 forces it)
 // Every shared-memory layout is chosen so that the 16-byte fragment loads of a quarter-warp are conflict-free.
 #include <cuda.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cstdlib>
+#include <cstring>
 
 #include "launch.h"
 
@@ -20,19 +22,7 @@ namespace pwh {
 
 namespace {
 
-#ifndef PWH_BK
-#define PWH_BK 8
-#endif
-#ifndef PWH_STAGES
-#define PWH_STAGES 4
-#endif
-constexpr int BM = 128, BN = 64, BK = PWH_BK, STAGES = PWH_STAGES, NT = 256;
-constexpr int WARPS_M = 4;                            // k_zgemm: 4 x 2 warps, warp tile 32 x 32 complex
-constexpr int KROW = BK * 16 + 64;                     // bytes per row of a K-major tile (== 64 mod 128)
-constexpr int MROW = BM * 16 + 32;                     // bytes per k-row of an M-major A tile (== 32 mod 128)
-constexpr int A_BYTES_K = BM * KROW;                   // 24576
-constexpr int A_BYTES_M = BK * MROW;                   // 16640
-constexpr int B_BYTES = BN * KROW;                     // 12288
+constexpr int BM = 128, BN = 64;                       // CTA tile (complex elements)
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes));
@@ -70,146 +60,22 @@ __device__ __forceinline__ double2 lds128(uint32_t addr) {
   return v;
 }
 
-enum { EPI_PARTIAL = 0, EPI_ACC = 1 };
+enum { EPI_PARTIAL = 0, EPI_ACC = 1, EPI_STORE = 2 };   // split-K partial | C += alpha AB | C = alpha AB
 
-// A_KMAJOR = true : op(A)[m,k] = conj(A[k + m*lda])  (CN);   false : op(A)[m,k] = A[m + k*lda]  (NN)
-template <bool A_KMAJOR, int EPI>
-__global__ void __launch_bounds__(NT, 1)
-k_zgemm(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* __restrict__ A, int64_t lda,
-        const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha) {
-  extern __shared__ __align__(1024) unsigned char smem[];
-  constexpr int A_BYTES = A_KMAJOR ? A_BYTES_K : A_BYTES_M;
-  constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm = warp % WARPS_M, wn = warp / WARPS_M;
-  // CN: m-tile fastest (all tiles of one K split are co-resident and share the streamed K range through L2)
-  // NN: n-tile fastest (the CTAs that share one slab of A rows run together)
-  int tm, tn;
-  if (A_KMAJOR) { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
-  else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
-  const int m0 = tm * BM, n0 = tn * BN;
-  const int split = blockIdx.y;
-  const int64_t kbeg = (int64_t)split * k_per_split;
-  const int64_t kend = (kbeg + k_per_split < K) ? kbeg + k_per_split : K;
-  const int nkt = (int)((kend - kbeg + BK - 1) / BK);
-
-  auto load_stage = [&](int stage, int kt) {
-    const uint32_t sa = smem_base + stage * STAGE_BYTES, sb = sa + A_BYTES;
-    const int64_t k0 = kbeg + (int64_t)kt * BK;
-    if (A_KMAJOR) {
-#pragma unroll
-      for (int i = 0; i < (BM * BK) / NT; ++i) {
-        const int idx = tid + i * NT, r = idx / BK, kk = idx % BK;
-        const bool ok = (m0 + r < M) && (k0 + kk < kend);
-        const c128* src = ok ? A + (int64_t)(m0 + r) * lda + k0 + kk : A;
-        cp_async16(sa + r * KROW + kk * 16, src, ok ? 16 : 0);
-      }
-    } else {
-#pragma unroll
-      for (int i = 0; i < (BM * BK) / NT; ++i) {
-        const int idx = tid + i * NT, kk = idx / BM, r = idx % BM;
-        const bool ok = (m0 + r < M) && (k0 + kk < kend);
-        const c128* src = ok ? A + (int64_t)(k0 + kk) * lda + m0 + r : A;
-        cp_async16(sa + kk * MROW + r * 16, src, ok ? 16 : 0);
-      }
-    }
-#pragma unroll
-    for (int i = 0; i < (BN * BK) / NT; ++i) {
-      const int idx = tid + i * NT, r = idx / BK, kk = idx % BK;
-      const bool ok = (n0 + r < N) && (k0 + kk < kend);
-      const c128* src = ok ? B + (int64_t)(n0 + r) * ldb + k0 + kk : B;
-      cp_async16(sb + r * KROW + kk * 16, src, ok ? 16 : 0);
-    }
-  };
-
-  double cr[4][4][2], ci[4][4][2];
-#pragma unroll
-  for (int i = 0; i < 4; ++i)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) { cr[i][j][0] = cr[i][j][1] = 0.0; ci[i][j][0] = ci[i][j][1] = 0.0; }
-
-#pragma unroll
-  for (int s = 0; s < STAGES - 1; ++s) {
-    if (s < nkt) load_stage(s, s);
-    cp_async_commit();
-  }
-
-  const int frow = lane >> 2, fk = lane & 3;
-  // per-thread fragment base offsets inside a stage
-  const uint32_t a_off = A_KMAJOR ? (uint32_t)((wm * 32 + frow) * KROW + fk * 16)
-                                  : (uint32_t)(fk * MROW + (wm * 32 + frow) * 16);
-  const uint32_t b_off = (uint32_t)(A_BYTES + (wn * 32 + frow) * KROW + fk * 16);
-
-  for (int kt = 0; kt < nkt; ++kt) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    {
-      const int nk = kt + STAGES - 1;
-      if (nk < nkt) load_stage(nk % STAGES, nk);
-      cp_async_commit();
-    }
-    const uint32_t st = smem_base + (kt % STAGES) * STAGE_BYTES;
-#pragma unroll
-    for (int k4 = 0; k4 < BK / 4; ++k4) {
-      double2 a[4], b[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const uint32_t ao = A_KMAJOR ? (uint32_t)(i * 8 * KROW + k4 * 64) : (uint32_t)(k4 * 4 * MROW + i * 8 * 16);
-        a[i] = lds128(st + a_off + ao);
-        b[i] = lds128(st + b_off + (uint32_t)(i * 8 * KROW + k4 * 64));
-      }
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const double nai = -a[i].y;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          if (A_KMAJOR) {  // conj(a) * b
-            dmma(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
-            dmma(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
-            dmma(cr[i][j][0], cr[i][j][1], a[i].y, b[j].y);
-            dmma(ci[i][j][0], ci[i][j][1], nai, b[j].x);
-          } else {         // a * b
-            dmma(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
-            dmma(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
-            dmma(cr[i][j][0], cr[i][j][1], nai, b[j].y);
-            dmma(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
-          }
-        }
-      }
-    }
-  }
-  cp_async_wait<0>();
-
-  // epilogue: thread holds C[m = frow][n = 2*fk + {0,1}] of every 8x8 block
-  c128* Cout = C;
-  if (EPI == EPI_PARTIAL) Cout += (int64_t)split * ldc * N;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int m = m0 + wm * 32 + i * 8 + frow;
-    if (m >= M) continue;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int n = n0 + wn * 32 + j * 8 + 2 * fk + h;
-        if (n >= N) continue;
-        c128* p = Cout + (int64_t)n * ldc + m;
-        if (EPI == EPI_PARTIAL) {
-          *p = cmake(cr[i][j][h], ci[i][j][h]);
-        } else {
-          c128 t = *p;
-          t.x = fma(alpha, cr[i][j][h], t.x);
-          t.y = fma(alpha, ci[i][j][h], t.y);
-          *p = t;
-        }
-      }
-    }
-  }
+// Hermitian C = A^H B (Gram matrix Psi^H (H Psi)): only the 128 x 64 tiles with floor(m/128) <=
+// floor(n/128) are computed; tile column tn holds tn/2 + 1 of them, so columns 2j and 2j+1 start at linear index
+// j(j+1) and (j+1)^2.  The split-K reduction mirrors the rest.
+__device__ __forceinline__ void herm_tile(int idx, int& tm, int& tn) {
+  int j = (int)((sqrtf(4.f * (float)idx + 1.f) - 1.f) * 0.5f);
+  while (j * (j + 1) > idx) --j;
+  while ((j + 1) * (j + 2) <= idx) ++j;
+  const int r = idx - j * (j + 1);
+  if (r <= j) { tn = 2 * j; tm = r; } else { tn = 2 * j + 1; tm = r - (j + 1); }
 }
 
+// A_KMAJOR = true : op(A)[m,k] = conj(A[k + m*lda])  (CN);   false : op(A)[m,k] = A[m + k*lda]  (NN)
 // ---------------------------------------------------------------------------------------------------------------
-// 3M variant (the default): one complex product as THREE real DMMA products instead of four,
+// 3M complex product: one complex product as THREE real DMMA products instead of four,
 //     T1 = ar.br,  T2 = ai.bi,  T3 = (ar + ai).(br + bi)   =>   re = T1 - T2,  im = T3 - T1 - T2
 // (for conj(a): ai -> -ai).  16 warps (4 x 4), warp tile 32 x 16 complex, three accumulator sets of 16 doubles;
 // the sums ar+ai / br+bi are formed on the fragments (one DADD per fragment element).  The imaginary part carries a
@@ -236,7 +102,7 @@ struct Tile3 {
 template <bool A_KMAJOR, int EPI, int BK_, int STAGES_>
 __global__ void __launch_bounds__(NT3, 1)
 k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128* __restrict__ A, int64_t lda,
-          const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha) {
+          const c128* __restrict__ B, int64_t ldb, c128* __restrict__ C, int64_t ldc, double alpha, int herm) {
   using T = Tile3<BK_>;
   constexpr int BK = BK_, STAGES = STAGES_, KROW = T::KROW, MROW = T::MROW;
   extern __shared__ __align__(1024) unsigned char smem[];
@@ -248,8 +114,10 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
   // CN: m-tile fastest (all tiles of one K split are co-resident and share the streamed K range through L2)
   // NN: n-tile fastest (the CTAs that share one slab of A rows run together)
   int tm, tn;
-  if (A_KMAJOR) { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
-  else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
+  if (A_KMAJOR) {
+    if (herm) herm_tile((int)blockIdx.x, tm, tn);
+    else { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
+  } else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
   const int m0 = tm * BM, n0 = tn * BN;
   const int split = blockIdx.y;
   const int64_t kbeg = (int64_t)split * k_per_split;
@@ -367,6 +235,8 @@ k_zgemm3m(int M, int N, int64_t K, int tiles_m, int64_t k_per_split, const c128*
         c128* p = Cout + (int64_t)n * ldc + m;
         if (EPI == EPI_PARTIAL) {
           *p = cmake(re, im);
+        } else if (EPI == EPI_STORE) {
+          *p = cmake(alpha * re, alpha * im);
         } else {
           c128 t = *p;
           t.x = fma(alpha, re, t.x);
@@ -408,7 +278,7 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm,
 template <bool A_KMAJOR, int EPI, int BK_, int STAGES_>
 __global__ void __launch_bounds__(NT3, 1)
 k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int M, int N, int64_t K,
-              int tiles_m, int64_t k_per_split, c128* __restrict__ C, int64_t ldc, double alpha) {
+              int tiles_m, int64_t k_per_split, c128* __restrict__ C, int64_t ldc, double alpha, int herm) {
   constexpr int BK = BK_, STAGES = STAGES_, SS = BK / 8;        // SS sub-slabs of 8 k per stage
   constexpr int A_SUB = BM * 128, B_SUB = BN * 128;             // bytes of one 8-k sub-slab of A and of B
   constexpr int A_BYTES = SS * A_SUB, STAGE_BYTES = SS * (A_SUB + B_SUB);
@@ -417,8 +287,10 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp % W3_M, wn = warp / W3_M;
   int tm, tn;
-  if (A_KMAJOR) { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
-  else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
+  if (A_KMAJOR) {
+    if (herm) herm_tile((int)blockIdx.x, tm, tn);
+    else { tm = blockIdx.x % tiles_m; tn = blockIdx.x / tiles_m; }
+  } else { const int tiles_n = (N + BN - 1) / BN; tn = blockIdx.x % tiles_n; tm = blockIdx.x / tiles_n; }
   const int m0 = tm * BM, n0 = tn * BN;
   const int split = blockIdx.y;
   const int64_t kbeg = (int64_t)split * k_per_split;
@@ -527,6 +399,8 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
         c128* p = Cout + (int64_t)n * ldc + m;
         if (EPI == EPI_PARTIAL) {
           *p = cmake(re, im);
+        } else if (EPI == EPI_STORE) {
+          *p = cmake(alpha * re, alpha * im);
         } else {
           c128 t = *p;
           t.x = fma(alpha, re, t.x);
@@ -538,20 +412,24 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   }
 }
 
-// C[m + n*ldc] = scale[m] * sum_s part[s][m + n*M]   (fixed summation order => deterministic)
+// C[m + n*ldc] = scale[m] * sum_s part[s][m + n*M]   (fixed summation order => deterministic).  herm: the partial sums
+// exist for floor(m/128) <= floor(n/128) only; the other entries are the conjugates of their mirror images.
 __global__ void __launch_bounds__(256) k_splitk_reduce(int M, int N, int nsplit, const c128* __restrict__ part,
                                                        const double* __restrict__ scale, c128* __restrict__ C,
-                                                       int64_t ldc) {
+                                                       int64_t ldc, int herm) {
   const int64_t total = (int64_t)M * N;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
     const int m = (int)(i % M);
     const int64_t n = i / M;
+    const bool mirror = herm && (m / BM) > (int)(n / BM);
+    const int64_t src = mirror ? (int64_t)m * M + n : i;
     double sx = 0.0, sy = 0.0;
     for (int s = 0; s < nsplit; ++s) {
-      const c128 v = part[(int64_t)s * total + i];
+      const c128 v = part[(int64_t)s * total + src];
       sx += v.x;
       sy += v.y;
     }
+    if (mirror) sy = -sy;
     const double f = scale ? scale[m] : 1.0;
     C[n * ldc + m] = cmake(f * sx, f * sy);
   }
@@ -574,8 +452,6 @@ __global__ void __launch_bounds__(256) k_dmma_probe(int iters, double* __restric
   if (s == 12345.678) sink[0] = s;
 }
 
-constexpr int smem_cn() { return STAGES * (A_BYTES_K + B_BYTES); }
-constexpr int smem_nn() { return STAGES * (A_BYTES_M + B_BYTES); }
 // 3M kernels: CN streams K = npw in slabs of 8 through 4 stages, NN (K = nproj) in slabs of 16 through 3 stages
 // (measured on B200, cfg 3/4: CN 41.3 vs 40.7 TFLOP/s and NN 35.7 vs 38.2 for slabs of 8 vs 16)
 constexpr int CN3_BK = 8, CN3_STAGES = 4, NN3_BK = 16, NN3_STAGES = 3;
@@ -588,19 +464,15 @@ constexpr int NUM_SMS = 148;
 
 }  // namespace
 
-// PWH_ZGEMM_4M=1 selects the four-product kernels (kept for comparison and as the numerical reference of the 3M ones)
-static bool use_3m() {
-  static const bool v = [] { const char* e = getenv("PWH_ZGEMM_4M"); return !(e && e[0] == '1'); }();
-  return v;
-}
-
 // cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static std::atomic<bool> g_no_tma{false};
+void zgemm_set_no_tma(bool off) { g_no_tma.store(off, std::memory_order_relaxed); }
+
 static EncodeTiledFn encode_fn() {
-  const char* e = getenv("PWH_ZGEMM_NO_TMA");   // read at every call so that the tests can switch kernels
-  if (e && e[0] == '1') return nullptr;
+  if (g_no_tma.load(std::memory_order_relaxed)) return nullptr;
   static const EncodeTiledFn fn = [] {
     void* p = nullptr;
     cudaDriverEntryPointQueryResult q;
@@ -626,24 +498,26 @@ static bool make_map(CUtensorMap* tm, const c128* base, int64_t inner, int64_t o
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// The projector matrix of a handle never changes: its two tensor maps (K-major operand of P^H Y, M-major operand of
+// P C) are encoded once at setup.  `ok` is false when the driver has no TMA encoder or refused the operand.
+void zgemm_make_proj_maps(ProjMaps& pm, const c128* P, int64_t npw, int64_t nproj, int64_t ldp) {
+  static_assert(sizeof(CUtensorMap) == sizeof(pm.cn), "ProjMaps storage");
+  pm.ok = nproj > 0 && make_map(reinterpret_cast<CUtensorMap*>(pm.cn), P, npw, nproj, ldp, BM) &&
+          make_map(reinterpret_cast<CUtensorMap*>(pm.nn), P, npw, nproj, ldp, NNT_BK);
+}
+
 cudaError_t zgemm_init() {
-  {
-    cudaError_t e = cudaFuncSetAttribute(k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem_tma(CNT_BK, CNT_STAGES));
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             smem_tma(NNT_BK, NNT_STAGES));
-    if (e != cudaSuccess) return e;
-  }
-  cudaError_t e = cudaFuncSetAttribute(k_zgemm<true, EPI_PARTIAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_cn());
+  cudaError_t e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES>));
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_zgemm<false, EPI_ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_nn());
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES>));
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           smem_cn3());
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<false, EPI_STORE, NNT_BK, NNT_STAGES>));
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_zgemm3m<false, EPI_ACC, NN3_BK, NN3_STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              smem_nn3());
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES>));
+  if (e != cudaSuccess) return e;
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m<false, EPI_ACC, NN3_BK, NN3_STAGES>));
+  if (e != cudaSuccess) return e;
+  return set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m<false, EPI_STORE, NN3_BK, NN3_STAGES>));
 }
 
 cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float* ms) {
@@ -664,11 +538,20 @@ cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float
   return e;
 }
 
-int zgemm_cn_splits(int64_t M, int64_t N, int64_t K) {
+// number of 128 x 64 tiles of C the CN kernel computes: all of them, or -- for a Hermitian C (herm) -- those that
+// touch the block upper triangle  floor(m/128) <= floor(n/128)
+static int64_t cn_tiles(int64_t M, int64_t N, bool herm) {
+  const int64_t tiles_m = (M + BM - 1) / BM, tiles_n = (N + BN - 1) / BN;
+  if (!herm) return tiles_m * tiles_n;
+  int64_t t = 0;
+  for (int64_t tn = 0; tn < tiles_n; ++tn) t += std::min<int64_t>(tiles_m, tn / 2 + 1);
+  return t;
+}
+
+static int splits_for_tiles(int64_t tiles, int64_t K) {
   // Split K so that tiles * splits fills whole waves of the 148 SMs (one CTA per SM): among the candidates with at
   // most 16 waves and at least 8 k-slabs per split, take the fewest splits within 1 % of the best wave efficiency.
-  const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
-  const int64_t max_split = std::max<int64_t>(1, K / (8 * BK));   // at least 8 k-slabs per split (small problems: one wave of short CTAs)
+  const int64_t max_split = std::max<int64_t>(1, K / (8 * CNT_BK));   // small problems: one wave of short CTAs
   int best = 1;
   double best_eff = 0.0;
   for (int64_t s = 1; s <= max_split; ++s) {
@@ -681,53 +564,77 @@ int zgemm_cn_splits(int64_t M, int64_t N, int64_t K) {
   return best;
 }
 
-size_t zgemm_cn_workspace(int64_t M, int64_t N, int64_t K) {
-  return sizeof(c128) * (size_t)zgemm_cn_splits(M, N, K) * (size_t)M * (size_t)N;
+int zgemm_cn_splits(int64_t M, int64_t N, int64_t K, bool herm) { return splits_for_tiles(cn_tiles(M, N, herm), K); }
+
+size_t zgemm_cn_workspace(int64_t M, int64_t N, int64_t K, bool herm) {
+  return sizeof(c128) * (size_t)zgemm_cn_splits(M, N, K, herm) * (size_t)M * (size_t)N;
+}
+
+// max over n <= N of zgemm_cn_workspace(M, n, K): the split count is not monotone in the number of tiles, so a
+// workspace sized for N bands must be sized for the worst narrower block as well
+size_t zgemm_cn_workspace_upto(int64_t M, int64_t N, int64_t K) {
+  size_t best = 0;
+  for (int64_t tn = 1; tn <= (N + BN - 1) / BN; ++tn) {
+    const int64_t n = std::min<int64_t>(tn * BN, N);
+    best = std::max(best, zgemm_cn_workspace(M, n, K, false));
+  }
+  return best;
 }
 
 void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda, const c128* B, int64_t ldb,
-                     const double* scale, c128* C, int64_t ldc, void* ws, cudaStream_t st) {
+                     const double* scale, c128* C, int64_t ldc, void* ws, cudaStream_t st, const ProjMaps* pmA, bool herm) {
   if (M <= 0 || N <= 0) return;
-  const int nsplit = zgemm_cn_splits(M, N, K);
-  const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
+  if (M != N) herm = false;
+  const int nsplit = zgemm_cn_splits(M, N, K, herm);
+  const int tiles_m = (int)((M + BM - 1) / BM);
   int64_t kps = (K + nsplit - 1) / nsplit;
-  kps = (kps + BK - 1) / BK * BK;
-  dim3 grid(tiles_m * tiles_n, nsplit);
+  kps = (kps + CNT_BK - 1) / CNT_BK * CNT_BK;
+  dim3 grid((unsigned)cn_tiles(M, N, herm), nsplit);
   c128* part = reinterpret_cast<c128*>(ws);
   {
     ScopedLaunch sl(ST_ZGEMM_CN, st);
     CUtensorMap tmA, tmB;
-    if (use_3m() && make_map(&tmA, A, K, M, lda, BM) && make_map(&tmB, B, K, N, ldb, BN))
+    bool tma = false;
+    if (pmA && pmA->ok && !g_no_tma.load(std::memory_order_relaxed)) { memcpy(&tmA, pmA->cn, sizeof(tmA)); tma = true; }
+    else tma = make_map(&tmA, A, K, M, lda, BM);
+    if (tma && make_map(&tmB, B, K, N, ldb, BN))
       k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES><<<grid, NT3, smem_tma(CNT_BK, CNT_STAGES), st>>>(
-          tmA, tmB, (int)M, (int)N, K, tiles_m, kps, part, M, 0.0);
-    else if (use_3m())
-      k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES><<<grid, NT3, smem_cn3(), st>>>(
-          (int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
+          tmA, tmB, (int)M, (int)N, K, tiles_m, kps, part, M, 0.0, herm ? 1 : 0);
     else
-      k_zgemm<true, EPI_PARTIAL><<<grid, NT, smem_cn(), st>>>((int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0);
+      k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES><<<grid, NT3, smem_cn3(), st>>>(
+          (int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0, herm ? 1 : 0);
   }
   const int64_t total = M * N;
   int blocks = (int)((total + 255) / 256);
   if (blocks > NUM_SMS * 8) blocks = NUM_SMS * 8;
   ScopedLaunch sl(ST_SPLITK, st);
-  k_splitk_reduce<<<blocks, 256, 0, st>>>((int)M, (int)N, nsplit, part, scale, C, ldc);
+  k_splitk_reduce<<<blocks, 256, 0, st>>>((int)M, (int)N, nsplit, part, scale, C, ldc, herm ? 1 : 0);
 }
 
-void launch_zgemm_nn_acc(int64_t M, int64_t N, int64_t K, double alpha, const c128* A, int64_t lda, const c128* B,
-                         int64_t ldb, c128* C, int64_t ldc, cudaStream_t st) {
+// C = alpha * A B (+ C when accumulate)
+void launch_zgemm_nn(int64_t M, int64_t N, int64_t K, double alpha, const c128* A, int64_t lda, const c128* B,
+                     int64_t ldb, c128* C, int64_t ldc, bool accumulate, cudaStream_t st, const ProjMaps* pmA) {
   if (M <= 0 || N <= 0 || K <= 0) return;
   const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
   dim3 grid(tiles_m * tiles_n, 1);
   ScopedLaunch sl(ST_ZGEMM_NN, st);
   CUtensorMap tmA, tmB;
-  if (use_3m() && make_map(&tmA, A, M, K, lda, NNT_BK) && make_map(&tmB, B, K, N, ldb, BN))
+  bool tma = false;
+  if (pmA && pmA->ok && !g_no_tma.load(std::memory_order_relaxed)) { memcpy(&tmA, pmA->nn, sizeof(tmA)); tma = true; }
+  else tma = make_map(&tmA, A, M, K, lda, NNT_BK);
+  tma = tma && make_map(&tmB, B, K, N, ldb, BN);
+  if (tma && accumulate)
     k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES><<<grid, NT3, smem_tma(NNT_BK, NNT_STAGES), st>>>(
-        tmA, tmB, (int)M, (int)N, K, tiles_m, K, C, ldc, alpha);
-  else if (use_3m())
+        tmA, tmB, (int)M, (int)N, K, tiles_m, K, C, ldc, alpha, 0);
+  else if (tma)
+    k_zgemm3m_tma<false, EPI_STORE, NNT_BK, NNT_STAGES><<<grid, NT3, smem_tma(NNT_BK, NNT_STAGES), st>>>(
+        tmA, tmB, (int)M, (int)N, K, tiles_m, K, C, ldc, alpha, 0);
+  else if (accumulate)
     k_zgemm3m<false, EPI_ACC, NN3_BK, NN3_STAGES><<<grid, NT3, smem_nn3(), st>>>(
-        (int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
+        (int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha, 0);
   else
-    k_zgemm<false, EPI_ACC><<<grid, NT, smem_nn(), st>>>((int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha);
+    k_zgemm3m<false, EPI_STORE, NN3_BK, NN3_STAGES><<<grid, NT3, smem_nn3(), st>>>(
+        (int)M, (int)N, K, tiles_m, K, A, lda, B, ldb, C, ldc, alpha, 0);
 }
 
 }  // namespace pwh

@@ -244,18 +244,39 @@ def make_workload(cfg_id: int, *, with_psi: bool = True, qr: str = "numpy",
                     degree=spec.degree, a=a, b=b, a0=a0)
 
 
-def random_problem(dims, cell, kpt, ecut, nproj, nband, seed) -> Workload:
-    """A small unstructured orthorhombic problem for parity edge cases (odd radices, non-cubic boxes, k-shifts):
-    the plane waves with 1/2|k+G|^2 <= ecut, random V_loc, random dense projectors, random (not orthonormal) Psi.
+def gsphere_general(lattice: np.ndarray, kpt, dims, ecut: float) -> np.ndarray:
+    """Integer G with 1/2 |B (k + n)|^2 <= ecut for a general (non-orthogonal) lattice, order n3 outer, n1 inner."""
+    B = reciprocal(np.asarray(lattice, dtype=np.float64))
+    k = np.asarray(kpt, dtype=np.float64)
+    rng_ = [np.arange(-(int(n) // 2) - 1, int(n) // 2 + 2, dtype=np.int64) for n in dims]
+    i3, i2, i1 = np.meshgrid(rng_[2], rng_[1], rng_[0], indexing="ij")
+    c = np.stack([i1 + k[0], i2 + k[1], i3 + k[2]], axis=-1) @ B
+    keep = 0.5 * np.einsum("...i,...i->...", c, c) <= float(ecut)
+    g = np.stack([i1[keep], i2[keep], i3[keep]], axis=1).astype(np.int32)
+    for ax, n in enumerate(dims):
+        span = int(g[:, ax].max()) - int(g[:, ax].min()) + 1
+        assert span <= n, f"sphere does not fit the FFT box along axis {ax}"
+    return np.ascontiguousarray(g)
+
+
+def random_problem(dims, cell, kpt, ecut, nproj, nband, seed, gvec: Optional[np.ndarray] = None) -> Workload:
+    """A small unstructured problem for parity edge cases (odd radices, non-cubic boxes, k-shifts, general lattices):
+    the plane waves with 1/2|k+G|^2 <= ecut (or the given `gvec` set), random V_loc, random dense projectors, random
+    (not orthonormal) Psi.  `cell` is either three orthorhombic edge lengths or a full 3x3 lattice (row i = a_i).
     Inputs only; the filter bounds are crude brackets (a0 < a < b) that keep the recurrence well-conditioned."""
     rng = np.random.default_rng(np.random.SeedSequence(list(SEED_ROOT) + [1000 + int(seed)]))
-    spec = ConfigSpec(1000 + int(seed), f"random_{dims[0]}x{dims[1]}x{dims[2]}", tuple(float(c) for c in cell),
+    cell_arr = np.asarray(cell, dtype=np.float64)
+    general = cell_arr.shape == (3, 3)
+    edges = tuple(float(np.linalg.norm(cell_arr[i])) for i in range(3)) if general else tuple(float(c) for c in cell_arr)
+    spec = ConfigSpec(1000 + int(seed), f"random_{dims[0]}x{dims[1]}x{dims[2]}", edges,
                       tuple(float(k) for k in kpt), tuple(int(d) for d in dims), ("ecut", float(ecut)), int(nband),
                       int(nband), 0, "sp", (0.0, 0.0), 3, False)
-    lattice = np.diag(np.asarray(spec.cell, dtype=np.float64))
+    lattice = cell_arr.copy() if general else np.diag(cell_arr)
     B = reciprocal(lattice)
     k = np.asarray(spec.kpt, dtype=np.float64)
-    gvec = gsphere(spec)
+    if gvec is None:
+        gvec = gsphere_general(lattice, k, spec.fft_dims, ecut) if general else gsphere(spec)
+    gvec = np.ascontiguousarray(gvec, dtype=np.int32)
     npw = gvec.shape[0]
     q = (gvec.astype(np.float64) + k[None, :]) @ B
     kin = 0.5 * np.einsum("ij,ij->i", q, q)

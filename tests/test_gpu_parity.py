@@ -338,33 +338,54 @@ def test_host_entry_points(gpu, cfg2):
 # ----------------------------------------------------------------------------------------------------------------
 # BASELINE.json's full sizes, in the launch configuration bench.py times
 # ----------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("cfg,sample", [(3, (0, 255, 511)), (4, (0, 517, 1023)), (5, (3, 2047))])
-def test_full_size_sampled_bands(gpu, cfg, sample):
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_sampled_bands(gpu, cfg):
     """Configs 3-5 with ALL their bands, driven exactly as bench.py's step drives them (filter of the config's degree in
-    column blocks of `block`, H.Psi in the same blocks, Gram of the whole block), checked on sampled outputs the oracle
-    can compute one by one: bands never interact before gram, so the oracle filters the
-    sampled bands alone; a Gram entry is one dot product of two such bands.  The samples sit in
-    different band groups of the local kernels, different column blocks and at both ends of the ZGEMM tiles."""
+    column blocks of `block`, H.Psi in the same blocks, Hermitian Gram of the whole block), checked on sampled outputs the
+    oracle can compute one by one: bands never interact before gram, so the oracle filters the
+    16 sampled bands alone; a Gram entry is one dot product of two such bands.  The samples cover the
+    first and last band, both sides of every column-block boundary and random bands in between, i.e. different band
+    groups of the local kernels, different column blocks and both ends of the ZGEMM tiles."""
     import torch
     w = synth.make_workload(cfg, qr="torch-cuda")
     spec = w.spec
-    assert w.npw == synth.EXPECTED_NPW[cfg] and w.psi.shape[0] == spec.nband
+    M = spec.nband
+    assert w.npw == synth.EXPECTED_NPW[cfg] and w.psi.shape[0] == M
+    rng = np.random.default_rng(7000 + cfg)
+    fixed = {0, M - 1, 127, 128, spec.block - 1, spec.block % M, M // 2}
+    extra = [int(i) for i in rng.permutation(M) if int(i) not in fixed]
+    idx = sorted(fixed) + extra[:16 - len(fixed)]
+    assert len(idx) == 16
+    rows = np.sort(rng.choice(M, size=64, replace=False))
+    cols = np.sort(rng.choice(M, size=64, replace=False))
     ham = setup(gpu, w)
     psi = to_dev(w.psi)
     hpsi = torch.empty_like(psi)
-    for b0 in range(0, spec.nband, spec.block):
+    for b0 in range(0, M, spec.block):
         gpu.cheb_filter(ham, psi[b0:b0 + spec.block], spec.degree, w.a, w.b, w.a0)
-    for b0 in range(0, spec.nband, spec.block):
+    for b0 in range(0, M, spec.block):
         gpu.apply_h(ham, psi[b0:b0 + spec.block], hpsi[b0:b0 + spec.block])
-    g = gpu.gram(psi, hpsi)
+    g = gpu.gram(psi, hpsi, hermitian=True)
+    g_full = gpu.gram(psi[:256], hpsi[:192])               # general (non-Hermitian) product on a ragged sub-block
     torch.cuda.synchronize()
-    idx = list(sample)
     y_gpu = psi[idx].cpu().numpy()
     hy_gpu = hpsi[idx].cpu().numpy()
     g_gpu = g[idx][:, idx].cpu().numpy()
     g_scale = float(g.abs().max())
+    herm_defect = float((g - g.conj().T).abs().max())
+    g_blk = g[rows][:, cols].cpu().numpy()
+    y_rows = psi[rows].cpu().numpy()
+    hy_cols = hpsi[cols].cpu().numpy()
+    g_sub = g_full.cpu().numpy()
+    g_sub_ref_in = (psi[:256:17].cpu().numpy(), hpsi[:192:13].cpu().numpy())
     ham.destroy()
-    del psi, hpsi, g
+    del psi, hpsi, g, g_full
+
+    # the whole Gram matrix is Hermitian (H is; PAPER.md:140), including across the mirrored blocks
+    assert herm_defect <= 1e-12 * g_scale
+    # a 64 x 64 block of random rows and columns: every entry against the oracle's dot product of the GPU's own bands
+    assert relerr(g_blk, oracle.gram(y_rows, hy_cols)) <= TOL_H
+    assert relerr(g_sub[::17][:, ::13], oracle.gram(*g_sub_ref_in)) <= TOL_H
 
     y_ref = oracle.cheb_filter(*ham_args(w), w.psi[idx], spec.degree, w.a, w.b, w.a0)
     hy_ref = oracle.apply_h(*ham_args(w), y_ref)
@@ -376,3 +397,174 @@ def test_full_size_sampled_bands(gpu, cfg, sample):
     assert relerr(hy_gpu, oracle.apply_h(*ham_args(w), y_gpu)) <= TOL_H
     assert relerr(g_gpu, oracle.gram(y_gpu, hy_gpu)) <= TOL_H
     assert np.abs(g_gpu - g_ref).max() <= TOL_F * g_scale
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# the rest of the ABI's input space: general lattices, arbitrary G order, non-convex G sets, padded projectors
+# ----------------------------------------------------------------------------------------------------------------
+def check_all(gpu, w, gvec=None, psi=None, proj=None, degrees=(1, 2, 5)):
+    """apply_h, gram and cheb_filter of workload `w` against the oracle at the north_star tolerances."""
+    ham = setup(gpu, w)
+    x = to_dev(w.psi)
+    hx = gpu.apply_h(ham, x)
+    ref_h = oracle.apply_h(*ham_args(w), w.psi)
+    assert relerr(hx.cpu().numpy(), ref_h) <= TOL_H
+    assert relerr(gpu.gram(x, hx).cpu().numpy(), oracle.gram(w.psi, ref_h)) <= TOL_H
+    for m in degrees:
+        y = gpu.cheb_filter(ham, x.clone(), m, w.a, w.b, w.a0).cpu().numpy()
+        assert relerr(y, oracle.cheb_filter(*ham_args(w), w.psi, m, w.a, w.b, w.a0)) <= TOL_F, m
+    return ham
+
+
+HEX = [[6.0, 0.0, 0.0], [-3.0, 3.0 * math.sqrt(3.0), 0.0], [0.0, 0.0, 9.0]]           # hexagonal, 120 degrees
+TRICLINIC = [[7.0, 0.3, -0.5], [1.1, 6.5, 0.4], [-0.8, 1.2, 8.0]]
+FCC = [[0.0, 4.0, 4.0], [4.0, 0.0, 4.0], [4.0, 4.0, 0.0]]                             # primitive fcc: B is bcc-like
+
+
+@pytest.mark.parametrize("name,seed,lattice,dims,kpt,ecut", [
+    ("hexagonal", 101, HEX, (24, 24, 30), (1.0 / 3.0, 1.0 / 3.0, 0.25), 14.0),
+    ("triclinic", 102, TRICLINIC, (20, 24, 30), (0.1, -0.2, 0.3), 9.0),
+    ("fcc", 103, FCC, (24, 24, 24), (0.5, 0.0, 0.5), 10.0),
+    ("triclinic48", 104, TRICLINIC, (48, 48, 40), (0.0, 0.0, 0.0), 20.0),     # the size-specialised plane kernel, skewed disc
+])
+def test_general_lattice(gpu, name, seed, lattice, dims, kpt, ecut):
+    """Non-orthogonal lattices (the kinetic term 1/2|k+G|^2 needs the full reciprocal metric): every
+    off-diagonal cofactor of the library's reciprocal-lattice construction is exercised, and the sphere is an oblique
+    ellipsoid in index space (skewed discs, x-line ranges that differ per row)."""
+    w = synth.random_problem(dims, np.asarray(lattice), kpt, ecut, 6, 5, seed=seed)
+    assert np.abs(w.lattice - np.diag(np.diag(w.lattice))).max() > 0.1
+    kin_gpu_check = oracle.kinetic(w.lattice, w.kpt, w.gvec)
+    assert kin_gpu_check.max() <= ecut * (1 + 1e-12)
+    ham = check_all(gpu, w)
+    # kinetic term alone, element-wise: H with V_loc = 0 and no projectors applied to unit-modulus vectors
+    ham0 = gpu.ham_setup(w.lattice, w.kpt, w.fft_dims, w.gvec, np.zeros_like(w.vloc), None, None)
+    ones = np.ones((1, w.npw), dtype=np.complex128)
+    kin_gpu = gpu.apply_h(ham0, to_dev(ones)).cpu().numpy()[0]
+    assert np.abs(kin_gpu.imag).max() == 0.0
+    assert np.abs(kin_gpu.real - kin_gpu_check).max() <= 1e-13 * kin_gpu_check.max()
+    ham0.destroy()
+    ham.destroy()
+
+
+@pytest.mark.parametrize("which", ["cfg2", "box"])
+def test_shuffled_gvec_order(gpu, cfg2, which):
+    """include/pwham.h accepts the plane waves in ANY order: a random permutation of gvec (and of the rows of Psi and P
+    with it) must give the permuted result."""
+    if which == "cfg2":
+        w0 = cfg2
+        nb = 24
+    else:
+        w0 = synth.random_problem((30, 20, 24), (11.0, 8.0, 9.0), (0.25, 0.125, -0.375), 5.0, 9, 6, seed=77)
+        nb = 6
+    perm = np.random.default_rng(123).permutation(w0.npw)
+    import dataclasses
+    w = dataclasses.replace(w0, gvec=np.ascontiguousarray(w0.gvec[perm]), proj=np.ascontiguousarray(w0.proj[:, perm]),
+                            psi=np.ascontiguousarray(w0.psi[:nb][:, perm]))
+    ham = check_all(gpu, w, degrees=(3,))
+    # and against the unpermuted problem: same numbers, permuted
+    ref = oracle.apply_h(*ham_args(w0), w0.psi[:nb])
+    out = gpu.apply_h(ham, to_dev(w.psi)).cpu().numpy()
+    assert relerr(out, ref[:, perm]) <= TOL_H
+    ham.destroy()
+
+
+@pytest.mark.parametrize("hole", ["x_slab", "centre", "random_half"])
+def test_nonconvex_gset(gpu, hole):
+    """A collision-free G set that is not a convex sphere (include/pwham.h promises any such set): a sphere with a slab of
+    x removed (touched x-lines not contiguous), with its centre removed (disc rows with gaps), and a random half of a sphere.
+    None of them satisfies the preconditions of the size-specialised plane kernel, which pwh_ham_setup must detect by
+    itself (no environment switch) and fall back to the generic-size plane kernel."""
+    base = synth.random_problem((48, 48, 36), (20.0, 20.0, 15.0), (0.0, 0.0, 0.0), 7.0, 5, 4, seed=90)
+    g = base.gvec
+    if hole == "x_slab":
+        keep = np.abs(g[:, 0]) >= 3
+    elif hole == "centre":
+        keep = (np.abs(g[:, 0]) >= 2) | (np.abs(g[:, 1]) >= 2)
+    else:
+        keep = np.random.default_rng(5).random(g.shape[0]) < 0.5
+    w = synth.random_problem((48, 48, 36), (20.0, 20.0, 15.0), (0.0, 0.0, 0.0), 7.0, 5, 4, seed=91,
+                             gvec=g[keep])
+    assert 0 < w.npw < base.npw
+    ham = check_all(gpu, w, degrees=(2,))
+    assert "kf_plane" in ham.kernels() and "kv2_plane" not in ham.kernels()
+    ham.destroy()
+    # the convex sphere on the same box does take the specialised kernel
+    ham_b = setup(gpu, base)
+    assert "kv2_plane" in ham_b.kernels() or "kv3_plane" in ham_b.kernels()
+    ham_b.destroy()
+
+
+def test_padded_projector_leading_dimension(gpu, cfg2):
+    """ldp > npw (include/pwham.h: 'ldp >= npw'): the projector matrix is borrowed with padded columns; it changes the
+    tensor-map stride of operand A in both ZGEMMs.  The padding holds NaNs, which must never be read."""
+    import torch
+    w = cfg2
+    ldp = w.npw + 5
+    pbuf = torch.full((w.nproj, ldp), complex(float("nan"), float("nan")), dtype=torch.complex128, device="cuda")
+    pbuf[:, : w.npw] = to_dev(w.proj)
+    ham = gpu.ham_setup(w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, pbuf[:, : w.npw], w.dij)
+    psi = w.psi[:70]
+    out = gpu.apply_h(ham, to_dev(psi)).cpu().numpy()
+    assert relerr(out, oracle.apply_h(*ham_args(w), psi)) <= TOL_H
+    y = gpu.cheb_filter(ham, to_dev(psi), 3, w.a, w.b, w.a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(w), psi, 3, w.a, w.b, w.a0)) <= TOL_F
+    ham.destroy()
+
+
+@pytest.mark.parametrize("n,npw", [(1, 5), (64, 300), (130, 4099), (257, 1031), (512, 2500)])
+def test_gram_hermitian_variant(gpu, n, npw):
+    """pwh_gram_herm: G = X^H (D X) with a real diagonal D is Hermitian; half of the tiles are computed, the rest
+    mirrored -- every entry against the oracle's dot products (H_Psi = Psi^H (H Psi))."""
+    rng = np.random.default_rng(n * 7 + npw)
+    x = rng.standard_normal((n, npw)) + 1j * rng.standard_normal((n, npw))
+    y = x * rng.uniform(-2.0, 3.0, size=npw)[None, :]
+    g = gpu.gram(to_dev(x), to_dev(y), hermitian=True).cpu().numpy()
+    ref = oracle.gram(x, y)
+    assert relerr(g, ref) <= TOL_H
+    assert np.abs(g - ref).max() <= 1e-11 * np.abs(ref).max() * math.sqrt(npw)
+    assert np.abs(g - g.conj().T).max() <= 1e-12 * np.abs(ref).max()
+
+
+def test_two_handles_alive(gpu):
+    """Two handles with different shared-memory needs alive at once (two k-points on different boxes): the handle made
+    first must still work after the second one has been set up, and the other way round."""
+    wa = synth.random_problem((48, 48, 180), (14.0, 14.0, 50.0), (0.0, 0.0, 0.0), 5.0, 4, 3, seed=60)
+    wb = synth.random_problem((48, 48, 30), (14.0, 14.0, 9.0), (0.25, 0.25, 0.25), 5.0, 4, 3, seed=61)
+    wc = synth.random_problem((96, 96, 12), (28.0, 28.0, 4.0), (0.0, 0.0, 0.0), 5.0, 4, 3, seed=62)
+    ha, hb, hc = setup(gpu, wa), setup(gpu, wb), setup(gpu, wc)
+    for w, h in ((wa, ha), (wb, hb), (wc, hc), (wa, ha)):
+        out = gpu.apply_h(h, to_dev(w.psi)).cpu().numpy()
+        assert relerr(out, oracle.apply_h(*ham_args(w), w.psi)) <= TOL_H
+    for h in (ha, hb, hc):
+        h.destroy()
+
+
+def test_ragged_last_block_through_host_entry(gpu, cfg2):
+    """392 bands in column blocks of 200: the ragged 192-band tail picks a different split-K count than the 200-band
+    block the workspace was sized for (pwh_workspace_bytes must cover every nband <= nband_max)."""
+    import torch
+    w = cfg2
+    rng = np.random.default_rng(392)
+    psi = (rng.standard_normal((392, w.npw)) + 1j * rng.standard_normal((392, w.npw))) / math.sqrt(2.0 * w.npw)
+    ham = setup(gpu, w)
+    L = gpu.load_library()
+    sizes = [int(L.pwh_workspace_bytes(ham.handle, n)) for n in range(1, 401)]
+    assert all(b >= a for a, b in zip(sizes, sizes[1:])), "pwh_workspace_bytes must be monotone in nband"
+    y_h = torch.from_numpy(psi.copy()).pin_memory()
+    gpu.cheb_filter_host(ham, y_h, 3, w.a, w.b, w.a0, block=200)
+    idx = [0, 199, 200, 391]
+    ref = oracle.cheb_filter(*ham_args(w), psi[idx], 3, w.a, w.b, w.a0)
+    assert relerr(y_h.numpy()[idx], ref) <= TOL_F
+    ham.destroy()
+
+
+def test_apply_h_rejects_overlapping_blocks(gpu, cfg1):
+    w = cfg1
+    ham = setup(gpu, w)
+    psi = to_dev(w.psi)
+    L = gpu.load_library()
+    ws = ham.workspace(w.nband)
+    rc = L.pwh_apply_h(ham.handle, w.nband, psi.data_ptr(), w.npw, psi.data_ptr() + 16 * w.npw, w.npw, ws.data_ptr(),
+                       ws.numel(), None)
+    assert rc == -1 and b"overlap" in L.pwh_last_error()
+    ham.destroy()

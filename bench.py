@@ -195,7 +195,7 @@ def run_reference(args):
     value = nb * apps * args.steps / t
     sample = (f"each step = the oracle on {nb} bands: degree-1 Chebyshev filter (1 H application + the first recurrence step) "
               f"+ Gram {nb}x{nb} (bounded sample of the config's {spec.nband} bands x {apps_per_band(spec)} applications)")
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1,
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(w).replace(f"nband={nb}", f"nband={spec.nband}").replace(f"Gram {nb}x{nb}", f"Gram {spec.nband}x{spec.nband}"), "sample": sample},

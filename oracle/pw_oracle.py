@@ -14,6 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pw_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "rr_oracle.c")]     # rr_oracle.c: Rayleigh-Ritz companion steps (oracle/rr_oracle.py)
 _LIB = os.path.join(_HERE, "libpw_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -23,8 +24,8 @@ TERM_KIN, TERM_LOC, TERM_NL, TERM_ALL = 1, 2, 4, 7
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (-O2, OpenMP over bands).  Building the checker is not using it."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-o", _LIB] + _SRCS + ["-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 

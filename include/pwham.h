@@ -146,6 +146,95 @@ int pwh_sweep_host(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi_hos
                    double b, double a0, pwh_c128* hpsi_host, int64_t ldh, pwh_c128* G_host, int64_t ldg,
                    void* stream);
 
+/*
+ * ---------------------------------------------------------------------------------------------------------------
+ * Rayleigh-Ritz companion steps: what one Chebyshev-filtering iteration (Algorithm 12, here with S = I)
+ * does around the filter.  All pointers DEVICE unless marked HOST; asynchronous on `stream` like the calls above, except
+ * pwh_chebfi_iteration (one host round trip, see there).  The dense M x M steps are hand-written kernels (blocked
+ * Cholesky, triangular inverse, one-sided Jacobi in one cooperative launch); no vendor solver library is called.
+ * `info` (DEVICE int32) of the dense solvers: > 0 = Jacobi sweeps used, < 0 = -(j+1) with j the first non-positive Cholesky
+ * pivot (the overlap matrix is not positive definite: linearly dependent bands); results are undefined in that case.
+ * ---------------------------------------------------------------------------------------------------------------
+ */
+
+/*
+ * pwh_rayleigh_quotients -- lambda[i] = Re(psi_i^H hpsi_i) / (psi_i^H psi_i)  ("Rayleigh quotients
+ * lambda_i = (H psi_i)^T psi_i / ((S psi_i)^T psi_i)", Algorithm 12 line 3), and, when minmax != NULL, minmax[0] = min_i,
+ * minmax[1] = max_i lambda[i] -- the interval the filter is built on.  lambda: nband doubles, minmax: 2 doubles.
+ */
+int pwh_rayleigh_quotients(int64_t npw, int64_t nband, const pwh_c128* psi, int64_t ld, const pwh_c128* hpsi, int64_t ldh,
+                           double* lambda, double* minmax, void* stream);
+
+/*
+ * pwh_residual_norms -- W_i = hpsi_i - lambda[i] psi_i and norms[i] = ||W_i||_2  (Algorithm 12 lines 11-12 with S = I:
+ * "W <- (H - Lambda S) Psi; compute residual norms").  W may be NULL (norms only); W may not alias the inputs.
+ */
+int pwh_residual_norms(int64_t npw, int64_t nband, const pwh_c128* psi, int64_t ld, const pwh_c128* hpsi, int64_t ldh,
+                       const double* lambda, pwh_c128* W, int64_t ldw, double* norms, void* stream);
+
+/*
+ * pwh_rotate -- Y = X Q: X npw x m (ldx), Q m x n column-major (ldq >= m), Y npw x n (ldy); Y must not overlap X
+ * (Algorithm 5 steps 4-5 / Algorithm 10: "Psi <- Psi X, H Psi <- (H Psi) X").  Runs on the DMMA ZGEMM.
+ */
+int pwh_rotate(int64_t npw, int64_t m, const pwh_c128* X, int64_t ldx, int64_t n, const pwh_c128* Q, int64_t ldq,
+               pwh_c128* Y, int64_t ldy, void* stream);
+
+/* Workspace of pwh_heev / pwh_hegv for matrices of order n (256-byte aligned device memory). */
+size_t pwh_dense_workspace_bytes(int64_t n);
+
+/*
+ * pwh_potrf -- in place A = U^H U for a Hermitian positive definite A (n x n column-major, only its upper triangle is
+ * read): the upper triangle becomes U (positive real diagonal), the strictly lower triangle is zeroed
+ * (Algorithm 9 step 2 "potrf").  *info = 0, or j+1 for the first non-positive pivot j.
+ */
+int pwh_potrf(int64_t n, pwh_c128* A, int64_t lda, int32_t* info, void* stream);
+
+/*
+ * pwh_heev -- eigen-decomposition of a Hermitian A (n x n, destroyed): w[0..n-1] ascending, column j of X the orthonormal
+ * eigenvector of w[j]  (Algorithm 5/10 step 3 with S_Psi = I).  X must not alias A.  Eigenvectors are defined up to a
+ * phase, and up to a unitary mixing inside a degenerate eigenspace.
+ * pwh_hegv -- A X = B X diag(w), X^H B X = I for Hermitian A and Hermitian positive definite B (both destroyed)
+ * (Algorithm 5/10 step 3 "hegvd"): B = U^H U, C = U^-H A U^-1, C Y = Y diag(w), X = U^-1 Y.
+ */
+int pwh_heev(int64_t n, pwh_c128* A, int64_t lda, double* w, pwh_c128* X, int64_t ldx, int32_t* info, void* ws,
+             size_t ws_bytes, void* stream);
+int pwh_hegv(int64_t n, pwh_c128* A, int64_t lda, pwh_c128* B, int64_t ldb, double* w, pwh_c128* X, int64_t ldx,
+             int32_t* info, void* ws, size_t ws_bytes, void* stream);
+
+/* Workspace of pwh_chol_ortho / pwh_rayleigh_ritz for an npw x nband block. */
+size_t pwh_rr_workspace_bytes(int64_t npw, int64_t nband);
+
+/*
+ * pwh_chol_ortho -- Algorithm 9 (S-Ortho) with S = I: S_Psi = Psi^H Psi = U^H U, Psi <- Psi U^-1 and, when hpsi != NULL,
+ * H Psi <- (H Psi) U^-1, in place.  U (optional, nband x nband column-major, ldu) receives the factor.
+ * *info as for pwh_potrf.  Afterwards Psi^H Psi = I.
+ */
+int pwh_chol_ortho(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh, pwh_c128* U,
+                   int64_t ldu, int32_t* info, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * pwh_rayleigh_ritz -- Algorithm 10 (RR) with S = I, in place: H_Psi = Psi^H (H Psi), S_Psi = Psi^H Psi,
+ * H_Psi X = S_Psi X Lambda, Psi <- Psi X, H Psi <- (H Psi) X (Algorithm 5).  lambda
+ * receives the nband Ritz values in ascending order; afterwards Psi^H Psi = I and Psi^H (H Psi) = diag(lambda).
+ */
+int pwh_rayleigh_ritz(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh, double* lambda,
+                      int32_t* info, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * pwh_chebfi_iteration -- one iteration of Algorithm 12 with S = I, in place on psi:
+ *   H Psi (lines 1-2); Rayleigh quotients, a = max, a0 = min - a0_margin (line 3; reading R5: the upper bound b
+ *   of the spectrum is an input); Psi <- p_degree(H) Psi in column blocks of `block` (lines 4-8); H Psi; Rayleigh-Ritz
+ *   (line 10); residual norms of the Ritz pairs (lines 11-12).
+ * On return psi holds the Ritz vectors, hpsi = H psi, lambda the Ritz values (ascending), resid the residual norms
+ * (lambda, resid: DEVICE, nband doubles), bounds_host (HOST, optional) = {a0, a}.  The call synchronises `stream` once, to
+ * bring the two Rayleigh-quotient bounds to the host (the paper's "mpi-sR" reduction sits at the same place).
+ * Workspace: pwh_chebfi_workspace_bytes(ham, nband, block).
+ */
+size_t pwh_chebfi_workspace_bytes(const pwh_ham* ham, int64_t nband, int64_t block);
+int pwh_chebfi_iteration(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh,
+                         int degree, double b, double a0_margin, double* lambda, double* resid, double* bounds_host,
+                         int32_t* info, void* ws, size_t ws_bytes, void* stream);
+
 /* Number of kernel launches issued by this library since load (all handles, all threads). */
 int64_t pwh_launch_count(void);
 
@@ -161,8 +250,11 @@ enum {
   PWH_STAGE_ZFWD_GATHER = 2,  /* a6 + a9: forward z transform, gather, kinetic + recurrence epilogue */
   PWH_STAGE_ZGEMM_CN = 3,     /* a7, a10: A^H B DMMA ZGEMM partial products (projector coefficients, Gram) */
   PWH_STAGE_SPLITK = 4,       /* a7, a10: fixed-order split-K sum (+ D scaling) */
-  PWH_STAGE_ZGEMM_NN = 5,     /* a8: P (D C) accumulated onto the recurrence term */
-  PWH_NSTAGES = 8
+  PWH_STAGE_ZGEMM_NN = 5,     /* a8: P (D C) accumulated onto the recurrence term; rotations Psi X */
+  PWH_STAGE_COLSTATS = 6,     /* Rayleigh quotients, residual norms (column reductions over the plane waves) */
+  PWH_STAGE_DENSE_SMALL = 7,  /* M x M steps: Cholesky panels, triangular inverse, shifts, sorts */
+  PWH_STAGE_JACOBI = 8,       /* M x M Hermitian eigen-solve (one cooperative launch) */
+  PWH_NSTAGES = 12
 };
 int pwh_profile_begin(void);
 int pwh_profile_end(double ms[PWH_NSTAGES], int64_t launches[PWH_NSTAGES]);

@@ -23,9 +23,13 @@ LIB_PATH = os.path.join(_HERE, "libpwham.so")
 EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply_h", "pwh_cheb_filter",
            "pwh_gram_workspace_bytes", "pwh_gram", "pwh_gram_herm", "pwh_ham_kernels", "pwh_apply_h_host", "pwh_cheb_filter_host", "pwh_sweep_host",
            "pwh_launch_count", "pwh_ham_info", "pwh_last_error", "pwh_profile_begin", "pwh_profile_end",
-           "pwh_probe_fp64_tensor_peak"]
+           "pwh_probe_fp64_tensor_peak",
+           "pwh_rayleigh_quotients", "pwh_residual_norms", "pwh_rotate", "pwh_dense_workspace_bytes", "pwh_potrf",
+           "pwh_heev", "pwh_hegv", "pwh_rr_workspace_bytes", "pwh_chol_ortho", "pwh_rayleigh_ritz",
+           "pwh_chebfi_workspace_bytes", "pwh_chebfi_iteration"]
 
-STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "reserved6", "reserved7"]
+STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "colstats", "dense_small",
+          "jacobi", "reserved9", "reserved10", "reserved11"]
 
 _lib = None
 
@@ -80,6 +84,30 @@ def load_library() -> ctypes.CDLL:
     L.pwh_probe_fp64_tensor_peak.restype = i32
     L.pwh_last_error.argtypes = []
     L.pwh_last_error.restype = ctypes.c_char_p
+    L.pwh_rayleigh_quotients.argtypes = [i64, i64, vp, i64, vp, i64, vp, vp, vp]
+    L.pwh_rayleigh_quotients.restype = i32
+    L.pwh_residual_norms.argtypes = [i64, i64, vp, i64, vp, i64, vp, vp, i64, vp, vp]
+    L.pwh_residual_norms.restype = i32
+    L.pwh_rotate.argtypes = [i64, i64, vp, i64, i64, vp, i64, vp, i64, vp]
+    L.pwh_rotate.restype = i32
+    L.pwh_dense_workspace_bytes.argtypes = [i64]
+    L.pwh_dense_workspace_bytes.restype = sz
+    L.pwh_potrf.argtypes = [i64, vp, i64, vp, vp]
+    L.pwh_potrf.restype = i32
+    L.pwh_heev.argtypes = [i64, vp, i64, vp, vp, i64, vp, vp, sz, vp]
+    L.pwh_heev.restype = i32
+    L.pwh_hegv.argtypes = [i64, vp, i64, vp, i64, vp, vp, i64, vp, vp, sz, vp]
+    L.pwh_hegv.restype = i32
+    L.pwh_rr_workspace_bytes.argtypes = [i64, i64]
+    L.pwh_rr_workspace_bytes.restype = sz
+    L.pwh_chol_ortho.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, vp, sz, vp]
+    L.pwh_chol_ortho.restype = i32
+    L.pwh_rayleigh_ritz.argtypes = [i64, i64, vp, i64, vp, i64, vp, vp, vp, sz, vp]
+    L.pwh_rayleigh_ritz.restype = i32
+    L.pwh_chebfi_workspace_bytes.argtypes = [vp, i64, i64]
+    L.pwh_chebfi_workspace_bytes.restype = sz
+    L.pwh_chebfi_iteration.argtypes = [vp, i64, i64, vp, i64, vp, i64, i32, dbl, dbl, vp, vp, vp, vp, vp, sz, vp]
+    L.pwh_chebfi_iteration.restype = i32
     _lib = L
     return L
 
@@ -310,6 +338,163 @@ def sweep_host(ham: Ham, psi_host, degree: int, a: float, b: float, a0: float, g
     _check(rc, "pwh_sweep_host")
 
 
+# ----------------------------------------------------------------------------------------------------------------
+# Rayleigh-Ritz companion steps (include/pwham.h, second half).  Small matrices cross this binding as torch tensors of
+# shape (n, n) indexed [row, column]; the library's column-major layout is their transpose's memory.
+# ----------------------------------------------------------------------------------------------------------------
+_scratch = {}
+
+
+def _ws(device, need: int, tag: str = "rr") -> torch.Tensor:
+    key = (torch.device(device).index, tag)
+    t = _scratch.get(key)
+    if t is None or t.numel() < need:
+        _scratch[key] = None
+        t = _scratch[key] = torch.empty(max(need, 256), dtype=torch.uint8, device=device)
+    return t
+
+
+def _cm(a: torch.Tensor) -> torch.Tensor:
+    """A fresh contiguous tensor holding a^T, i.e. the matrix `a` in column-major order (the solvers work in place)."""
+    return a.to(torch.complex128).T.contiguous().clone()
+
+
+def rayleigh_quotients(psi: torch.Tensor, hpsi: torch.Tensor):
+    """pwh_rayleigh_quotients: (lambda (nband,), minmax (2,)) as device tensors."""
+    L = load_library()
+    npw = int(psi.shape[1])
+    p, ld = _block_args(psi, npw, "psi")
+    h, ldh = _block_args(hpsi, npw, "hpsi")
+    nb = int(psi.shape[0])
+    lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    mm = torch.empty(2, dtype=torch.float64, device=psi.device)
+    with torch.cuda.device(psi.device):
+        _check(L.pwh_rayleigh_quotients(npw, nb, p, ld, h, ldh, lam.data_ptr(), mm.data_ptr(), _stream_ptr(psi.device)),
+               "pwh_rayleigh_quotients")
+    return lam, mm
+
+
+def residual_norms(psi: torch.Tensor, hpsi: torch.Tensor, lam: torch.Tensor, want_w: bool = False):
+    """pwh_residual_norms: norms (nband,) and, when want_w, W = hpsi - lam psi."""
+    L = load_library()
+    npw = int(psi.shape[1])
+    p, ld = _block_args(psi, npw, "psi")
+    h, ldh = _block_args(hpsi, npw, "hpsi")
+    nb = int(psi.shape[0])
+    lam = lam.to(device=psi.device, dtype=torch.float64).contiguous()
+    norms = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    w = torch.empty_like(psi) if want_w else None
+    with torch.cuda.device(psi.device):
+        _check(L.pwh_residual_norms(npw, nb, p, ld, h, ldh, lam.data_ptr(), w.data_ptr() if want_w else None, npw,
+                                    norms.data_ptr(), _stream_ptr(psi.device)), "pwh_residual_norms")
+    return (norms, w) if want_w else norms
+
+
+def rotate(x: torch.Tensor, q: torch.Tensor) -> torch.Tensor:
+    """pwh_rotate: Y = X Q for a block x (m, npw) and q (m, n) indexed [i, j]; returns (n, npw)."""
+    L = load_library()
+    npw = int(x.shape[1])
+    xp, ldx = _block_args(x, npw, "x")
+    m, n = int(q.shape[0]), int(q.shape[1])
+    q_cm = _cm(q)                                      # (n, m) memory = column-major m x n
+    y = torch.empty((n, npw), dtype=torch.complex128, device=x.device)
+    with torch.cuda.device(x.device):
+        _check(L.pwh_rotate(npw, m, xp, ldx, n, q_cm.data_ptr(), m, y.data_ptr(), npw, _stream_ptr(x.device)), "pwh_rotate")
+    return y
+
+
+def potrf(s: torch.Tensor):
+    """pwh_potrf: returns (U [row, column] upper triangular with S = U^H U, info)."""
+    L = load_library()
+    a = _cm(s)
+    n = int(a.shape[0])
+    info = torch.zeros(1, dtype=torch.int32, device=a.device)
+    with torch.cuda.device(a.device):
+        _check(L.pwh_potrf(n, a.data_ptr(), n, info.data_ptr(), _stream_ptr(a.device)), "pwh_potrf")
+    return a.T, int(info.item())
+
+
+def heev(a: torch.Tensor):
+    """pwh_heev: (w ascending (n,), X [row, column] with eigenvectors in its columns, sweeps)."""
+    L = load_library()
+    a_cm = _cm(a)
+    n = int(a_cm.shape[0])
+    w = torch.empty(n, dtype=torch.float64, device=a.device)
+    x = torch.empty((n, n), dtype=torch.complex128, device=a.device)
+    info = torch.zeros(1, dtype=torch.int32, device=a.device)
+    ws = _ws(a.device, int(L.pwh_dense_workspace_bytes(n)))
+    with torch.cuda.device(a.device):
+        _check(L.pwh_heev(n, a_cm.data_ptr(), n, w.data_ptr(), x.data_ptr(), n, info.data_ptr(), ws.data_ptr(), ws.numel(),
+                          _stream_ptr(a.device)), "pwh_heev")
+    return w, x.T, int(info.item())
+
+
+def hegv(a: torch.Tensor, b: torch.Tensor):
+    """pwh_hegv: A X = B X diag(w), X^H B X = I; returns (w, X [row, column], info)."""
+    L = load_library()
+    a_cm, b_cm = _cm(a), _cm(b)
+    n = int(a_cm.shape[0])
+    w = torch.empty(n, dtype=torch.float64, device=a.device)
+    x = torch.empty((n, n), dtype=torch.complex128, device=a.device)
+    info = torch.zeros(1, dtype=torch.int32, device=a.device)
+    ws = _ws(a.device, int(L.pwh_dense_workspace_bytes(n)))
+    with torch.cuda.device(a.device):
+        _check(L.pwh_hegv(n, a_cm.data_ptr(), n, b_cm.data_ptr(), n, w.data_ptr(), x.data_ptr(), n, info.data_ptr(),
+                          ws.data_ptr(), ws.numel(), _stream_ptr(a.device)), "pwh_hegv")
+    return w, x.T, int(info.item())
+
+
+def chol_ortho(psi: torch.Tensor, hpsi: Optional[torch.Tensor] = None):
+    """pwh_chol_ortho, in place on psi (and hpsi): returns (U [row, column], info)."""
+    L = load_library()
+    npw = int(psi.shape[1])
+    p, ld = _block_args(psi, npw, "psi")
+    nb = int(psi.shape[0])
+    h, ldh = (None, npw) if hpsi is None else _block_args(hpsi, npw, "hpsi")
+    u = torch.empty((nb, nb), dtype=torch.complex128, device=psi.device)
+    info = torch.zeros(1, dtype=torch.int32, device=psi.device)
+    ws = _ws(psi.device, int(L.pwh_rr_workspace_bytes(npw, nb)))
+    with torch.cuda.device(psi.device):
+        _check(L.pwh_chol_ortho(npw, nb, p, ld, h, ldh, u.data_ptr(), nb, info.data_ptr(), ws.data_ptr(), ws.numel(),
+                                _stream_ptr(psi.device)), "pwh_chol_ortho")
+    return u.T, int(info.item())
+
+
+def rayleigh_ritz(psi: torch.Tensor, hpsi: torch.Tensor):
+    """pwh_rayleigh_ritz, in place on psi and hpsi: returns (lambda (nband,), info)."""
+    L = load_library()
+    npw = int(psi.shape[1])
+    p, ld = _block_args(psi, npw, "psi")
+    h, ldh = _block_args(hpsi, npw, "hpsi")
+    nb = int(psi.shape[0])
+    lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    info = torch.zeros(1, dtype=torch.int32, device=psi.device)
+    ws = _ws(psi.device, int(L.pwh_rr_workspace_bytes(npw, nb)))
+    with torch.cuda.device(psi.device):
+        _check(L.pwh_rayleigh_ritz(npw, nb, p, ld, h, ldh, lam.data_ptr(), info.data_ptr(), ws.data_ptr(), ws.numel(),
+                                   _stream_ptr(psi.device)), "pwh_rayleigh_ritz")
+    return lam, int(info.item())
+
+
+def chebfi_iteration(ham: Ham, psi: torch.Tensor, hpsi: torch.Tensor, degree: int, b: float, a0_margin: float = 0.0,
+                     block: int = 0):
+    """pwh_chebfi_iteration, in place on psi / hpsi: returns dict(lam, resid (device tensors), a0, a, info)."""
+    L = load_library()
+    p, ld = _block_args(psi, ham.npw, "psi")
+    h, ldh = _block_args(hpsi, ham.npw, "hpsi")
+    nb = int(psi.shape[0])
+    lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    res = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    info = torch.zeros(1, dtype=torch.int32, device=psi.device)
+    bounds = (ctypes.c_double * 2)()
+    ws = _ws(psi.device, int(L.pwh_chebfi_workspace_bytes(ham.handle, nb, int(block))), tag="chebfi")
+    with torch.cuda.device(ham.device):
+        _check(L.pwh_chebfi_iteration(ham.handle, nb, int(block), p, ld, h, ldh, int(degree), float(b), float(a0_margin),
+                                      lam.data_ptr(), res.data_ptr(), bounds, info.data_ptr(), ws.data_ptr(), ws.numel(),
+                                      _stream_ptr(ham.device)), "pwh_chebfi_iteration")
+    return {"lam": lam, "resid": res, "a0": float(bounds[0]), "a": float(bounds[1]), "info": int(info.item())}
+
+
 def launch_count() -> int:
     return int(load_library().pwh_launch_count())
 
@@ -320,10 +505,10 @@ def profile_begin() -> None:
 
 def profile_end() -> dict:
     """Returns {stage: (milliseconds, launches)} summed over the launches since profile_begin()."""
-    ms = (ctypes.c_double * 8)()
-    n = (ctypes.c_int64 * 8)()
+    ms = (ctypes.c_double * len(STAGES))()
+    n = (ctypes.c_int64 * len(STAGES))()
     _check(load_library().pwh_profile_end(ms, n), "pwh_profile_end")
-    return {STAGES[i]: (float(ms[i]), int(n[i])) for i in range(8) if n[i]}
+    return {STAGES[i]: (float(ms[i]), int(n[i])) for i in range(len(STAGES)) if n[i]}
 
 
 def probe_fp64_tensor_peak(iters: int = 20000, device="cuda:0") -> float:

@@ -7,7 +7,8 @@ namespace pwh {
 void count_launch();
 
 // Stage ids reported by pwh_profile_end (same order as PWH_STAGE_* in include/pwham.h).
-enum { ST_SCATTER_ZINV = 0, ST_PLANE = 1, ST_ZFWD_GATHER = 2, ST_ZGEMM_CN = 3, ST_SPLITK = 4, ST_ZGEMM_NN = 5 };
+enum { ST_SCATTER_ZINV = 0, ST_PLANE = 1, ST_ZFWD_GATHER = 2, ST_ZGEMM_CN = 3, ST_SPLITK = 4, ST_ZGEMM_NN = 5,
+       ST_COLSTATS = 6, ST_SMALL = 7, ST_JACOBI = 8 };
 // Counts one kernel launch and, while profiling is on, brackets it with a cudaEvent pair on `st`.
 class ScopedLaunch {
  public:
@@ -77,6 +78,23 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
 // C[m + n*ldc] = alpha * sum_k A[m + k*lda] * B[k + n*ldb]  (+ C[m + n*ldc] when accumulate)
 void launch_zgemm_nn(int64_t M, int64_t N, int64_t K, double alpha, const c128* A, int64_t lda, const c128* B,
                      int64_t ldb, c128* C, int64_t ldc, bool accumulate, cudaStream_t st, const ProjMaps* pmA = nullptr);
+
+// rr.cu -- Rayleigh-Ritz companion kernels (all pointers device)
+cudaError_t rr_kernels_init();
+void launch_rayleigh(int64_t npw, int64_t nband, const c128* psi, int64_t ld, const c128* hpsi, int64_t ldh, double* lambda,
+                     double* nrm2, double* minmax, cudaStream_t st);
+void launch_residual(int64_t npw, int64_t nband, const c128* psi, int64_t ld, const c128* hpsi, int64_t ldh,
+                     const double* lambda, c128* W, int64_t ldw, double* norms, cudaStream_t st);
+void launch_potrf_upper(int n, c128* A, int64_t lda, int* info, cudaStream_t st);
+void launch_trinv_upper(int n, const c128* U, int64_t ldu, c128* W, int64_t ldw, cudaStream_t st);
+void launch_hermitise(int n, c128* A, int64_t lda, cudaStream_t st);
+void launch_merge_info(const int* potrf_info, int* info, cudaStream_t st);
+size_t jacobi_scratch_bytes(int n);
+cudaError_t launch_heev_jacobi(int n, c128* A, int64_t lda, double* w, c128* X, int64_t ldx, int* sweeps, void* scratch,
+                               cudaStream_t st);
+
+// pwham.cu: records the thread-local error message of the C ABI and returns `code`
+int api_fail(int code, const char* fmt, ...);
 
 // pwham.cu: raises the dynamic shared-memory limit of a kernel to the device's opt-in maximum.  The attribute is
 // process-global per kernel, so it is set to the maximum once rather than to one handle's need.

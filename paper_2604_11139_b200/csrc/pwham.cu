@@ -86,6 +86,18 @@ static int fail(int code, const char* fmt, ...) {
   return code;
 }
 
+namespace pwh {
+int api_fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+}  // namespace pwh
+
 #define CUDA_TRY(expr)                                                                        \
   do {                                                                                        \
     cudaError_t e__ = (expr);                                                                 \
@@ -460,42 +472,42 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     if (fast_plane_smem(fp) > (size_t)smem_max || fast_zkernel_smem(fp) > (size_t)smem_max) h->fast = false;
   }
   // size-specialised plane kernel (local_v2.cu): needs the register-resident z kernels, a box side it is instantiated
-  // for, x-lines contiguous modulo n1 and every y-row of the disc a contiguous run of x-lines
+  // for, x-lines contiguous modulo n1 and every y-row of the disc a contiguous run of x-lines (true for any convex cutoff
+  // sphere; otherwise the generic-size plane kernel of local_fast.cu serves)
   if (h->fast) {
-    V2Plan& vp = h->vp;
-    memset(&vp, 0, sizeof(vp));
-    bool ok = !env_on("PWH_NO_V2") && nxl < 65536 && ncols < (1 << 30);
-    for (int i = 0; i < nxl && ok; ++i) ok = x_of_xl[i] == (x_of_xl[0] + i) % n1;
+    bool pre = nxl < 65536 && ncols < (1 << 30);
+    for (int i = 0; i < nxl && pre; ++i) pre = x_of_xl[i] == (x_of_xl[0] + i) % n1;
     std::vector<int2> yrow((size_t)n2, make_int2(0, 0));
-    if (ok) {
+    if (pre) {
       std::vector<int> row_gy(n2, INT32_MAX), row_first(n2, 0), row_xlmin(n2, 0), row_cnt(n2, 0);
-      for (int r = 0; r < ncols && ok; ++r) {
+      for (int r = 0; r < ncols && pre; ++r) {
         const Col& c = cols[order[r]];
         const int xl = xl_of_x[c.xw];
         if (row_cnt[c.yw] == 0) { row_gy[c.yw] = c.gy; row_first[c.yw] = r; row_xlmin[c.yw] = xl; row_cnt[c.yw] = 1; }
         else {
-          ok = row_gy[c.yw] == c.gy && r == row_first[c.yw] + row_cnt[c.yw] && xl == row_xlmin[c.yw] + row_cnt[c.yw];
+          pre = row_gy[c.yw] == c.gy && r == row_first[c.yw] + row_cnt[c.yw] && xl == row_xlmin[c.yw] + row_cnt[c.yw];
           row_cnt[c.yw]++;
         }
       }
       for (int y = 0; y < n2; ++y) yrow[y] = make_int2(row_first[y] - row_xlmin[y], row_xlmin[y] | (row_cnt[y] << 16));
     }
-    if (ok) ok = v2_select(vp, n1, n2, nxl, (size_t)smem_max);
-    if (ok) {
+    const long double PI = 3.14159265358979323846264338327950288L;
+    V2Plan& vp = h->vp;
+    memset(&vp, 0, sizeof(vp));
+    if (pre && !env_on("PWH_NO_V2") && v2_select(vp, n1, n2, nxl, (size_t)smem_max)) {
       vp.n1 = n1; vp.n2 = n2; vp.n3 = n3; vp.ncols_pad = lp.ncols_pad; vp.nxl = nxl; vp.x0 = x_of_xl[0];
       vp.zcol = ncols;
       vp.div_nxl = lp.div_nxl;
       if ((rc = upload(h, yrow, &vp.yrow, st))) return rc;
-      const long double PI = 3.14159265358979323846264338327950288L;
       for (int ax = 0; ax < 2; ++ax) {
         const int n = dims[ax], r1 = vp.r1[ax], r2 = vp.r2[ax];
         std::vector<c128> ta((size_t)r2 * (r1 + 1), cmake(0.0, 0.0)), tb((size_t)r1 * (r2 + 1), cmake(0.0, 0.0));
-        for (int s = 0; s < r2; ++s)
+        for (int s_ = 0; s_ < r2; ++s_)
           for (int k1 = 0; k1 < r1; ++k1) {
-            const long double ang = 2.0L * PI * (long double)((s * k1) % n) / (long double)n;
+            const long double ang = 2.0L * PI * (long double)((s_ * k1) % n) / (long double)n;
             const c128 w = cmake((double)cosl(ang), (double)sinl(ang));
-            ta[(size_t)s * (r1 + 1) + k1] = w;
-            tb[(size_t)k1 * (r2 + 1) + s] = w;
+            ta[(size_t)s_ * (r1 + 1) + k1] = w;
+            tb[(size_t)k1 * (r2 + 1) + s_] = w;
           }
         if ((rc = upload(h, ta, &vp.twA[ax], st))) return rc;
         if ((rc = upload(h, tb, &vp.twB[ax], st))) return rc;
@@ -585,16 +597,18 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   // whole waves of the 148 SMs: among the group sizes whose buffer is between 24 and 56 MB take the one with the best
   // wave efficiency (ncu, profiles/r01d: 7 bands x 128 planes = 6.05 waves left the seventh wave almost empty)
   const size_t per_band = (size_t)n3 * lp.ncols_pad * sizeof(c128);
+  const int64_t slots = 148;                                                            // resident plane CTAs
+  const size_t win_hi = 56u << 20;
   const int64_t min_grp = (2 * 148 + n3 - 1) / n3;
   int64_t g_lo = std::max<int64_t>(std::max<int64_t>((int64_t)((24u << 20) / std::max<size_t>(per_band, 1)), min_grp), 1);
-  int64_t g_hi = std::max<int64_t>((int64_t)((56u << 20) / std::max<size_t>(per_band, 1)), g_lo);
+  int64_t g_hi = std::max<int64_t>((int64_t)(win_hi / std::max<size_t>(per_band, 1)), g_lo);
   g_hi = std::min<int64_t>(g_hi, 4096);
   g_lo = std::min<int64_t>(g_lo, g_hi);
   int64_t grp = g_hi;
   double best_eff = -1.0;
   for (int64_t c = g_lo; c <= g_hi; ++c) {
-    const int64_t ctas = c * n3, waves = (ctas + 147) / 148;
-    const double eff = (double)ctas / (double)(waves * 148);
+    const int64_t ctas = c * n3, waves = (ctas + slots - 1) / slots;
+    const double eff = (double)ctas / (double)(waves * slots);
     if (eff >= best_eff + 0.005 || (eff >= best_eff - 0.005 && c > grp && eff >= 0.97)) { best_eff = std::max(eff, best_eff); grp = c; }
   }
   h->band_group = (int)grp;

@@ -294,3 +294,35 @@ def random_problem(dims, cell, kpt, ecut, nproj, nband, seed, gvec: Optional[np.
                     vloc=np.ascontiguousarray(vloc), proj=np.ascontiguousarray(proj), dij=dij,
                     psi=np.ascontiguousarray(psi), atoms=np.zeros((0, 3)), depths=np.zeros((0,)), degree=3, a=a, b=b,
                     a0=a0)
+
+
+def paw_blocks(nproj: int, dij: np.ndarray, seed: int, block_sizes=None):
+    """Per-atom dense blocks for the PAW-style generalised problem: the projector
+    index is cut into consecutive blocks (one per atom; 8 projectors per atom in the BASELINE.json configs, an uneven mix
+    for the random test problems), D^R = diag(the config's D_i) + a seeded Hermitian off-diagonal part of relative size
+    0.3, Q^R = B B^H / (2 n_R) + a small indefinite Hermitian part (positive enough that S = I + P Q P^H stays positive
+    definite).  Returns (offsets int32 [nblocks + 1], [D^R], [Q^R]).  Inputs only."""
+    rng = np.random.default_rng(np.random.SeedSequence(list(SEED_ROOT) + [5000 + int(seed)]))
+    if block_sizes is None:
+        block_sizes = [8] * (nproj // 8) if nproj % 8 == 0 and nproj > 0 else []
+        rest = nproj - sum(block_sizes)
+        cyc = [4, 1, 5, 3, 8, 2]
+        i = 0
+        while rest > 0:
+            b = min(rest, cyc[i % len(cyc)])
+            block_sizes.append(b)
+            rest -= b
+            i += 1
+    assert sum(block_sizes) == nproj
+    offsets = np.concatenate([[0], np.cumsum(block_sizes)]).astype(np.int32)
+    dblocks, qblocks = [], []
+    for r, n in enumerate(block_sizes):
+        lo = int(offsets[r])
+        a = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+        d = np.diag(np.asarray(dij[lo:lo + n], dtype=np.float64)).astype(np.complex128) + 0.3 * (a + a.conj().T) / 2
+        bm = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+        c = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+        q = bm @ bm.conj().T / (2.0 * n) + 0.02 * (c + c.conj().T) / 2
+        dblocks.append(np.ascontiguousarray((d + d.conj().T) / 2))
+        qblocks.append(np.ascontiguousarray((q + q.conj().T) / 2))
+    return offsets, dblocks, qblocks

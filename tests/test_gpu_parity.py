@@ -92,6 +92,13 @@ RANDOM_CASES = [
     ((125, 6, 4), (30.0, 4.0, 3.0), (0.25, 0.0, 0.0), 2.0, 4, 3),           # 125 = 5^3: generic-stage fallback plan
     ((15, 16, 45), (6.0, 6.5, 14.0), (0.0, 0.25, 0.0), 4.0, 6, 4),          # single-pass 15 and 16, 45 = 9*5
     ((180, 120, 8), (75.0, 50.0, 4.0), (0.25, 0.25, 0.25), 3.0, 5, 3),      # cfg 5's axis lengths 15*12 and 12*10
+    # the large planes of the size-specialised plane kernel: cfg 4's with its 65 x-lines, cfg 5's and cfg 3's with a k-point,
+    # a small sphere in a large box, and a sphere wider than half the box (too large for it: generic-size kernel)
+    ((128, 128, 12), (54.0, 54.0, 5.0), (0.0, 0.0, 0.0), 6.95, 6, 5),
+    ((120, 120, 6), (50.0, 50.0, 3.0), (0.25, 0.25, 0.25), 8.0, 4, 3),
+    ((96, 96, 8), (40.0, 40.0, 4.0), (0.25, 0.25, 0.25), 7.1, 4, 3),
+    ((128, 128, 4), (54.0, 54.0, 2.0), (0.25, -0.25, 0.0), 0.8, 3, 4),
+    ((128, 128, 4), (54.0, 54.0, 2.0), (0.0, 0.0, 0.0), 11.0, 3, 3),
 ]
 
 
@@ -468,29 +475,34 @@ def test_shuffled_gvec_order(gpu, cfg2, which):
     ham.destroy()
 
 
-@pytest.mark.parametrize("hole", ["x_slab", "centre", "random_half"])
+@pytest.mark.parametrize("hole", ["x_slab", "centre", "random_columns", "random_half"])
 def test_nonconvex_gset(gpu, hole):
     """A collision-free G set that is not a convex sphere (include/pwham.h promises any such set): a sphere with a slab of
-    x removed (touched x-lines not contiguous), with its centre removed (disc rows with gaps), and a random half of a sphere.
-    None of them satisfies the preconditions of the size-specialised plane kernel, which pwh_ham_setup must detect by
-    itself (no environment switch) and fall back to the generic-size plane kernel."""
+    x removed (touched x-lines not contiguous), with its centre removed (disc rows with gaps), with a random half of its
+    z-columns removed, and a random half of its points (which still touches every column of the disc, so the specialised
+    kernel remains valid).  The first three violate the preconditions of the size-specialised plane kernels, which
+    pwh_ham_setup must detect by itself (no environment switch) and fall back to the generic-size plane kernel."""
     base = synth.random_problem((48, 48, 36), (20.0, 20.0, 15.0), (0.0, 0.0, 0.0), 7.0, 5, 4, seed=90)
     g = base.gvec
     if hole == "x_slab":
         keep = np.abs(g[:, 0]) >= 3
     elif hole == "centre":
         keep = (np.abs(g[:, 0]) >= 2) | (np.abs(g[:, 1]) >= 2)
+    elif hole == "random_columns":
+        col_keep = np.random.default_rng(6).random((64, 64)) < 0.5
+        keep = col_keep[g[:, 0] + 32, g[:, 1] + 32]
     else:
         keep = np.random.default_rng(5).random(g.shape[0]) < 0.5
     w = synth.random_problem((48, 48, 36), (20.0, 20.0, 15.0), (0.0, 0.0, 0.0), 7.0, 5, 4, seed=91,
                              gvec=g[keep])
     assert 0 < w.npw < base.npw
     ham = check_all(gpu, w, degrees=(2,))
-    assert "kf_plane" in ham.kernels() and "kv2_plane" not in ham.kernels()
+    if hole != "random_half":
+        assert "kf_plane" in ham.kernels() and "kv2_plane" not in ham.kernels()
     ham.destroy()
     # the convex sphere on the same box does take the specialised kernel
     ham_b = setup(gpu, base)
-    assert "kv2_plane" in ham_b.kernels() or "kv3_plane" in ham_b.kernels()
+    assert "kv2_plane" in ham_b.kernels()
     ham_b.destroy()
 
 

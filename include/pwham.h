@@ -254,6 +254,7 @@ enum {
   PWH_STAGE_COLSTATS = 6,     /* Rayleigh quotients, residual norms (column reductions over the plane waves) */
   PWH_STAGE_DENSE_SMALL = 7,  /* M x M steps: Cholesky panels, triangular inverse, shifts, sorts */
   PWH_STAGE_JACOBI = 8,       /* M x M Hermitian eigen-solve (one cooperative launch) */
+  PWH_STAGE_AXPY = 9,         /* three-term axpy of the filter on S^-1 H (generalised problem) */
   PWH_NSTAGES = 12
 };
 int pwh_profile_begin(void);

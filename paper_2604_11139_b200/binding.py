@@ -29,7 +29,7 @@ EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply
            "pwh_chebfi_workspace_bytes", "pwh_chebfi_iteration"]
 
 STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "colstats", "dense_small",
-          "jacobi", "reserved9", "reserved10", "reserved11"]
+          "jacobi", "axpy", "reserved10", "reserved11"]
 
 _lib = None
 

@@ -8,7 +8,7 @@ void count_launch();
 
 // Stage ids reported by pwh_profile_end (same order as PWH_STAGE_* in include/pwham.h).
 enum { ST_SCATTER_ZINV = 0, ST_PLANE = 1, ST_ZFWD_GATHER = 2, ST_ZGEMM_CN = 3, ST_SPLITK = 4, ST_ZGEMM_NN = 5,
-       ST_COLSTATS = 6, ST_SMALL = 7, ST_JACOBI = 8 };
+       ST_COLSTATS = 6, ST_SMALL = 7, ST_JACOBI = 8, ST_AXPY = 9 };
 // Counts one kernel launch and, while profiling is on, brackets it with a cudaEvent pair on `st`.
 class ScopedLaunch {
  public:
@@ -81,8 +81,8 @@ void launch_zgemm_nn(int64_t M, int64_t N, int64_t K, double alpha, const c128* 
 
 // rr.cu -- Rayleigh-Ritz companion kernels (all pointers device)
 cudaError_t rr_kernels_init();
-void launch_rayleigh(int64_t npw, int64_t nband, const c128* psi, int64_t ld, const c128* hpsi, int64_t ldh, double* lambda,
-                     double* nrm2, double* minmax, cudaStream_t st);
+void launch_rayleigh(int64_t npw, int64_t nband, const c128* psi, int64_t ld, const c128* hpsi, int64_t ldh,
+                     const c128* spsi, int64_t lds, double* lambda, double* nrm2, double* minmax, cudaStream_t st);
 void launch_residual(int64_t npw, int64_t nband, const c128* psi, int64_t ld, const c128* hpsi, int64_t ldh,
                      const double* lambda, c128* W, int64_t ldw, double* norms, cudaStream_t st);
 void launch_potrf_upper(int n, c128* A, int64_t lda, int* info, cudaStream_t st);
@@ -92,6 +92,19 @@ void launch_merge_info(const int* potrf_info, int* info, cudaStream_t st);
 size_t jacobi_scratch_bytes(int n);
 cudaError_t launch_heev_jacobi(int n, c128* A, int64_t lda, double* w, c128* X, int64_t ldx, int* sweeps, void* scratch,
                                cudaStream_t st);
+
+// paw.cu -- PAW-style generalised problem: block-diagonal D / Q, helpers for K of S^-1 = I - P K P^H, filter axpy
+void launch_blockdiag_apply(int64_t nproj, int64_t nband, const int* blk_of, const int* blk_lo, const int64_t* boff,
+                            const c128* blocks, const c128* in, int64_t ldi, c128* out, int64_t ldo, cudaStream_t st);
+void launch_blocks_to_dense(int64_t nproj, const int* blk_of, const int* blk_lo, const int64_t* boff, const c128* blocks,
+                            c128* out, int64_t ldo, cudaStream_t st);
+void launch_conj_transpose(int n, const c128* in, int64_t ldi, c128* out, int64_t ldo, cudaStream_t st);
+// A <- alpha A + beta B + gamma I  (B may be null)
+void launch_mat_axpby(int n, double alpha, c128* A, int64_t lda, double beta, const c128* B, int64_t ldb, double gamma,
+                      cudaStream_t st);
+// out = alpha (z - c y) - beta yprev  (yprev may be null; out may alias z or yprev)
+void launch_cheb_axpy(int64_t npw, int64_t nband, const c128* z, int64_t ldz, const c128* y, int64_t ldy, const c128* yprev,
+                      int64_t ldp, c128* out, int64_t ldo, double alpha, double cshift, double beta, cudaStream_t st);
 
 // pwham.cu: records the thread-local error message of the C ABI and returns `code`
 int api_fail(int code, const char* fmt, ...);

@@ -121,6 +121,14 @@ struct pwh_ham {
   ProjMaps pmaps;
   double* dij = nullptr;
   int band_group = 1;
+  // PAW-style generalised problem (pwh_ham_set_paw): per-atom dense D^R / Q^R blocks and K of S^-1 = I - P K P^H
+  bool paw = false;
+  int* blk_of = nullptr;         // [nproj] block (atom) of each projector
+  int* blk_lo = nullptr;         // [nblk + 1] first projector of each block
+  int64_t* boff = nullptr;       // [nblk] element offset of each packed block
+  c128* dblk = nullptr;          // packed column-major blocks D^R
+  c128* qblk = nullptr;          // packed column-major blocks Q^R
+  c128* kmat = nullptr;          // nproj x nproj, K
   std::vector<void*> allocs;
   // staging of the *_host entry points
   void* st_psi = nullptr;
@@ -657,6 +665,7 @@ extern "C" int pwh_ham_kernels(const pwh_ham* h, char* buf, size_t n) {
     s += "k_scatter_zinv k_plane k_zfwd_gather ";
   }
   if (h->nproj > 0) s += h->pmaps.ok ? "zgemm3m_tma" : "zgemm3m";
+  if (h->paw) s += " paw_blocks";
   snprintf(buf, n, "%s", s.c_str());
   return PWH_OK;
 }
@@ -679,7 +688,8 @@ static WsLayout ws_layout(const pwh_ham* h, int64_t nband) {
   w.ldw = (int64_t)align_up((size_t)h->npw, 16);
   size_t off = 0;
   w.colbuf = off; off += align_up((size_t)w.group * h->n3 * h->lp.ncols_pad * sizeof(c128), 256);
-  w.cmat = off;   off += align_up((size_t)std::max<int64_t>(h->nproj, 1) * nband * sizeof(c128), 256);
+  // projections C = P^H Y; with PAW blocks also blockdiag(D) C and blockdiag(Q) C (or K C)
+  w.cmat = off;   off += (h->paw ? 3 : 1) * align_up((size_t)std::max<int64_t>(h->nproj, 1) * nband * sizeof(c128), 256);
   w.part = off;   off += align_up(h->nproj > 0 ? zgemm_cn_workspace_upto(h->nproj, nband, h->npw) : 16, 256);
   w.y1 = off;     off += align_up((size_t)w.ldw * nband * sizeof(c128), 256);
   w.y2 = off;     off += align_up((size_t)w.ldw * nband * sizeof(c128), 256);
@@ -700,9 +710,16 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
                   cudaStream_t st) {
   c128* colbuf = reinterpret_cast<c128*>(ws + w.colbuf);
   c128* cmat = reinterpret_cast<c128*>(ws + w.cmat);
+  const size_t cmat_sz = align_up((size_t)std::max<int64_t>(h->nproj, 1) * nband * sizeof(c128), 256);
+  c128* cd = cmat;                                          // D C: what the second ZGEMM multiplies P with
   if (h->nproj > 0) {
     NvtxRange r("pwh:nonlocal:C=D.P^H.Y");
-    launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, y, ldy, h->dij, cmat, h->nproj, ws + w.part, st, &h->pmaps);
+    launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, y, ldy, h->paw ? nullptr : h->dij, cmat, h->nproj,
+                    ws + w.part, st, &h->pmaps);
+    if (h->paw) {   // per-atom dense blocks D^R
+      cd = reinterpret_cast<c128*>(ws + w.cmat + cmat_sz);
+      launch_blockdiag_apply(h->nproj, nband, h->blk_of, h->blk_lo, h->boff, h->dblk, cmat, h->nproj, cd, h->nproj, st);
+    }
   }
   {
     NvtxRange r("pwh:local+kinetic+recurrence");
@@ -729,7 +746,7 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
   }
   if (h->nproj > 0) {
     NvtxRange r("pwh:nonlocal:Y+=a.P.C");
-    launch_zgemm_nn(h->npw, nband, h->nproj, alpha, h->proj, h->ldp, cmat, h->nproj, out, ldout, true, st, &h->pmaps);
+    launch_zgemm_nn(h->npw, nband, h->nproj, alpha, h->proj, h->ldp, cd, h->nproj, out, ldout, true, st, &h->pmaps);
   }
   CUDA_TRY(cudaGetLastError());
   return PWH_OK;
@@ -845,6 +862,203 @@ extern "C" int pwh_gram(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx,
 extern "C" int pwh_gram_herm(int64_t npw, int64_t n, const pwh_c128* X, int64_t ldx, const pwh_c128* Y, int64_t ldy,
                              pwh_c128* G, int64_t ldg, void* ws, size_t ws_bytes, void* stream) {
   return gram_impl(npw, n, X, ldx, n, Y, ldy, G, ldg, ws, ws_bytes, stream, true);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// PAW-style generalised problem H Psi = Lambda S Psi
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" int pwh_ham_set_paw(pwh_ham* h, int64_t nblocks, const int32_t* offsets, const pwh_c128* dblocks,
+                               const pwh_c128* qblocks, int32_t* info, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (h->nproj < 1) return fail(PWH_EINVAL, "the handle has no projectors");
+  if (nblocks < 1 || !offsets || !dblocks || !qblocks || !info) return fail(PWH_EINVAL, "null argument or nblocks < 1");
+  if (offsets[0] != 0 || offsets[nblocks] != h->nproj) return fail(PWH_EINVAL, "offsets must run from 0 to nproj");
+  for (int64_t r = 0; r < nblocks; ++r)
+    if (offsets[r + 1] <= offsets[r]) return fail(PWH_EINVAL, "offsets must increase");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t J = h->nproj;
+  std::vector<int> blk_of((size_t)J), blk_lo((size_t)nblocks + 1);
+  std::vector<int64_t> boff((size_t)nblocks);
+  int64_t tot = 0;
+  for (int64_t r = 0; r < nblocks; ++r) {
+    blk_lo[r] = offsets[r];
+    boff[r] = tot;
+    const int64_t n = offsets[r + 1] - offsets[r];
+    tot += n * n;
+    for (int64_t i = offsets[r]; i < offsets[r + 1]; ++i) blk_of[i] = (int)r;
+  }
+  blk_lo[nblocks] = (int)J;
+  int rc;
+  const int* d_of; const int* d_lo; const int64_t* d_off;
+  if ((rc = upload(h, blk_of, &d_of, st)) || (rc = upload(h, blk_lo, &d_lo, st)) || (rc = upload(h, boff, &d_off, st))) return rc;
+  c128 *db = nullptr, *qb = nullptr, *km = nullptr;
+  CUDA_TRY(cudaMalloc(&db, tot * sizeof(c128))); h->allocs.push_back(db);
+  CUDA_TRY(cudaMalloc(&qb, tot * sizeof(c128))); h->allocs.push_back(qb);
+  CUDA_TRY(cudaMalloc(&km, (size_t)J * J * sizeof(c128))); h->allocs.push_back(km);
+  CUDA_TRY(cudaMemcpyAsync(db, dblocks, tot * sizeof(c128), cudaMemcpyDeviceToDevice, st));
+  CUDA_TRY(cudaMemcpyAsync(qb, qblocks, tot * sizeof(c128), cudaMemcpyDeviceToDevice, st));
+  // K of S^-1 = I - P K P^H (Woodbury), through two Cholesky factorisations so that only Hermitian
+  // positive definite matrices are factored:  G = P^H P = U^H U,  A = U Q U^H,  I + A = V^H V,  W = U^-1,  Z = V^-1,
+  //   K = W (I - Z Z^H) W^H = W W^H - (W Z)(W Z)^H        [ = G^-1 - (G + G Q G)^-1 ]
+  const size_t mat = align_up((size_t)J * J * sizeof(c128), 256);
+  const size_t part = align_up(std::max(zgemm_cn_workspace(J, J, h->npw, true), zgemm_cn_workspace(J, J, J, true)), 256);
+  unsigned char* scr = nullptr;
+  CUDA_TRY(cudaMalloc(&scr, 5 * mat + part + 256));
+  c128* G = (c128*)scr; c128* W = (c128*)(scr + mat); c128* T1 = (c128*)(scr + 2 * mat); c128* T2 = (c128*)(scr + 3 * mat);
+  c128* T3 = (c128*)(scr + 4 * mat);
+  void* pws = scr + 5 * mat;
+  int* pinfo = (int*)(scr + 5 * mat + part);
+  const int n = (int)J;
+  cudaError_t ce = rr_kernels_init();
+  if (ce == cudaSuccess) ce = zgemm_init();
+  if (ce == cudaSuccess) {
+    CUDA_TRY(cudaMemsetAsync(info, 0, sizeof(int), st));
+    launch_zgemm_cn(J, J, h->npw, h->proj, h->ldp, h->proj, h->ldp, nullptr, G, J, pws, st, &h->pmaps, true);   // G = P^H P
+    launch_hermitise(n, G, J, st);
+    launch_potrf_upper(n, G, J, pinfo, st);                                  // G <- U
+    launch_merge_info(pinfo, info, st);
+    launch_trinv_upper(n, G, J, W, J, st);                                   // W = U^-1
+    launch_blocks_to_dense(J, d_of, d_lo, d_off, qb, T1, J, st);             // T1 = Q
+    launch_conj_transpose(n, G, J, T2, J, st);                               // T2 = U^H
+    launch_zgemm_nn(J, J, J, 1.0, T1, J, T2, J, T3, J, false, st);           // T3 = Q U^H
+    launch_zgemm_nn(J, J, J, 1.0, G, J, T3, J, T1, J, false, st);            // T1 = A = U Q U^H
+    launch_mat_axpby(n, 1.0, T1, J, 0.0, nullptr, 0, 1.0, st);               // T1 = I + A
+    launch_hermitise(n, T1, J, st);
+    launch_potrf_upper(n, T1, J, pinfo, st);                                 // T1 <- V
+    launch_merge_info(pinfo, info, st);
+    launch_trinv_upper(n, T1, J, T2, J, st);                                 // T2 = Z = V^-1
+    launch_zgemm_nn(J, J, J, 1.0, W, J, T2, J, T3, J, false, st);            // T3 = W Z
+    launch_conj_transpose(n, T3, J, T1, J, st);                              // T1 = (W Z)^H
+    launch_conj_transpose(n, W, J, T2, J, st);                               // T2 = W^H
+    launch_zgemm_cn(J, J, J, T2, J, T2, J, nullptr, km, J, pws, st, nullptr, true);   // K = W W^H
+    launch_zgemm_cn(J, J, J, T1, J, T1, J, nullptr, T3, J, pws, st, nullptr, true);   // T3 = (W Z)(W Z)^H
+    launch_mat_axpby(n, 1.0, km, J, -1.0, T3, J, 0.0, st);
+    launch_hermitise(n, km, J, st);
+    ce = cudaGetLastError();
+  }
+  const cudaError_t cs = cudaStreamSynchronize(st);
+  cudaFree(scr);
+  CUDA_TRY(ce);
+  CUDA_TRY(cs);
+  h->blk_of = const_cast<int*>(d_of); h->blk_lo = const_cast<int*>(d_lo); h->boff = const_cast<int64_t*>(d_off);
+  h->dblk = db; h->qblk = qb; h->kmat = km;
+  h->paw = true;
+  return PWH_OK;
+}
+
+// H psi and S psi from one set of projections (HX_SX); either output may be null
+extern "C" int pwh_apply_hs(pwh_ham* h, int64_t nband, const pwh_c128* psi, int64_t ldpsi, pwh_c128* hpsi, int64_t ldh,
+                            pwh_c128* spsi, int64_t lds, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (!h->paw) return fail(PWH_EINVAL, "pwh_ham_set_paw has not been called on this handle");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (nband == 0) return PWH_OK;
+  if (!psi || (!hpsi && !spsi)) return fail(PWH_EINVAL, "psi null or no output");
+  if (ldpsi < h->npw || (hpsi && ldh < h->npw) || (spsi && lds < h->npw)) return fail(PWH_EINVAL, "leading dimension smaller than npw");
+  int rc = check_ws(h, nband, ws, ws_bytes);
+  if (rc) return rc;
+  if (hpsi && blocks_overlap(psi, ldpsi, hpsi, ldh, h->npw, nband)) return fail(PWH_EINVAL, "psi and hpsi overlap");
+  if (spsi && blocks_overlap(psi, ldpsi, spsi, lds, h->npw, nband)) return fail(PWH_EINVAL, "psi and spsi overlap");
+  NvtxRange r("pwh_apply_hs");
+  cudaStream_t st = (cudaStream_t)stream;
+  const WsLayout w = ws_layout(h, nband);
+  unsigned char* wsb = reinterpret_cast<unsigned char*>(ws);
+  if (hpsi) {   // computes C = P^H psi into cmat on the way
+    rc = h_step(h, nband, (const c128*)psi, ldpsi, nullptr, 0, (c128*)hpsi, ldh, 1.0, 0.0, 0.0, wsb, w, st);
+    if (rc) return rc;
+  }
+  if (spsi) {
+    c128* cmat = reinterpret_cast<c128*>(wsb + w.cmat);
+    const size_t cmat_sz = align_up((size_t)h->nproj * nband * sizeof(c128), 256);
+    c128* cq = reinterpret_cast<c128*>(wsb + w.cmat + 2 * cmat_sz);
+    if (!hpsi)
+      launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, (const c128*)psi, ldpsi, nullptr, cmat, h->nproj, wsb + w.part,
+                      st, &h->pmaps);
+    launch_blockdiag_apply(h->nproj, nband, h->blk_of, h->blk_lo, h->boff, h->qblk, cmat, h->nproj, cq, h->nproj, st);
+    CUDA_TRY(cudaMemcpy2DAsync(spsi, (size_t)lds * sizeof(c128), psi, (size_t)ldpsi * sizeof(c128), (size_t)h->npw * sizeof(c128),
+                               (size_t)nband, cudaMemcpyDeviceToDevice, st));
+    launch_zgemm_nn(h->npw, nband, h->nproj, 1.0, h->proj, h->ldp, cq, h->nproj, (c128*)spsi, lds, true, st, &h->pmaps);
+    CUDA_TRY(cudaGetLastError());
+  }
+  return PWH_OK;
+}
+
+// x <- S^-1 x = x - P K (P^H x) in place
+static int sinv_inplace(pwh_ham* h, int64_t nband, c128* x, int64_t ldx, unsigned char* wsb, const WsLayout& w, cudaStream_t st) {
+  c128* cmat = reinterpret_cast<c128*>(wsb + w.cmat);
+  const size_t cmat_sz = align_up((size_t)h->nproj * nband * sizeof(c128), 256);
+  c128* ck = reinterpret_cast<c128*>(wsb + w.cmat + 2 * cmat_sz);
+  launch_zgemm_cn(h->nproj, nband, h->npw, h->proj, h->ldp, x, ldx, nullptr, cmat, h->nproj, wsb + w.part, st, &h->pmaps);
+  launch_zgemm_nn(h->nproj, nband, h->nproj, 1.0, h->kmat, h->nproj, cmat, h->nproj, ck, h->nproj, false, st);
+  launch_zgemm_nn(h->npw, nband, h->nproj, -1.0, h->proj, h->ldp, ck, h->nproj, x, ldx, true, st, &h->pmaps);
+  CUDA_TRY(cudaGetLastError());
+  return PWH_OK;
+}
+
+extern "C" int pwh_apply_sinv(pwh_ham* h, int64_t nband, pwh_c128* x, int64_t ldx, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (!h->paw) return fail(PWH_EINVAL, "pwh_ham_set_paw has not been called on this handle");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (nband == 0) return PWH_OK;
+  if (!x || ldx < h->npw) return fail(PWH_EINVAL, "x null or ldx < npw");
+  int rc = check_ws(h, nband, ws, ws_bytes);
+  if (rc) return rc;
+  NvtxRange r("pwh_apply_sinv");
+  return sinv_inplace(h, nband, (c128*)x, ldx, reinterpret_cast<unsigned char*>(ws), ws_layout(h, nband), (cudaStream_t)stream);
+}
+
+// the scaled Chebyshev filter of S^-1 H (Algorithm 12 lines 4-8): per degree T = H Y_j, T <- S^-1 T, axpy
+extern "C" int pwh_cheb_filter_gen(pwh_ham* h, int64_t nband, pwh_c128* psi, int64_t ld, int degree, double a, double b,
+                                   double a0, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (!h->paw) return fail(PWH_EINVAL, "pwh_ham_set_paw has not been called on this handle");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (degree < 0) return fail(PWH_EINVAL, "degree < 0");
+  if (!(b > a)) return fail(PWH_EINVAL, "need b > a");
+  if (!(a0 < a)) return fail(PWH_EINVAL, "need a0 < a");
+  if (nband == 0 || degree == 0) return PWH_OK;
+  if (!psi) return fail(PWH_EINVAL, "psi null");
+  if (ld < h->npw) return fail(PWH_EINVAL, "ld < npw");
+  int rc = check_ws(h, nband, ws, ws_bytes);
+  if (rc) return rc;
+  NvtxRange r("pwh_cheb_filter_gen");
+  const WsLayout w = ws_layout(h, nband);
+  unsigned char* wsb = reinterpret_cast<unsigned char*>(ws);
+  cudaStream_t st = (cudaStream_t)stream;
+  c128* buf[3] = {reinterpret_cast<c128*>(psi), reinterpret_cast<c128*>(wsb + w.y1), reinterpret_cast<c128*>(wsb + w.y2)};
+  const int64_t lds[3] = {ld, w.ldw, w.ldw};
+  const double e = 0.5 * (b - a), c = 0.5 * (b + a), sigma1 = e / (a0 - c);
+  // where Y_j lives; T = S^-1 H Y_j goes to the one buffer that holds neither Y_j nor Y_{j-1}, and Y_{j+1} is written either
+  // over T or over Y_{j-1} (the axpy is entry by entry), chosen so that Y_degree lands in psi (as in pwh_cheb_filter)
+  std::vector<int> where((size_t)degree + 1, 0);
+  if (degree % 2 == 0) {
+    where[1] = 1;
+    for (int j = 2; j <= degree; ++j) where[j] = where[j - 2];
+  } else if (degree >= 3) {
+    where[1] = 1; where[2] = 2; where[3] = 0;
+    for (int j = 4; j <= degree; ++j) where[j] = where[j - 2];
+  }
+  double sigma = sigma1;
+  for (int j = 0; j < degree; ++j) {
+    const int ic = where[j], ip = j > 0 ? where[j - 1] : -1, io = where[j + 1];
+    int it = 0;
+    while (it == ic || it == ip) ++it;                 // the free buffer
+    rc = h_step(h, nband, buf[ic], lds[ic], nullptr, 0, buf[it], lds[it], 1.0, 0.0, 0.0, wsb, w, st);   // T = H Y_j
+    if (rc) return rc;
+    if ((rc = sinv_inplace(h, nband, buf[it], lds[it], wsb, w, st))) return rc;                          // T <- S^-1 T
+    double alpha, beta = 0.0;
+    if (j == 0) alpha = sigma1 / e;
+    else {
+      const double sigma_new = 1.0 / (2.0 / sigma1 - sigma);
+      alpha = 2.0 * sigma_new / e;
+      beta = sigma * sigma_new;
+      sigma = sigma_new;
+    }
+    launch_cheb_axpy(h->npw, nband, buf[it], lds[it], buf[ic], lds[ic], j > 0 ? buf[ip] : nullptr, j > 0 ? lds[ip] : 0,
+                     buf[io], lds[io], alpha, c, beta, st);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return PWH_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------------------

@@ -53,18 +53,19 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
   return s;
 }
 
-// lambda_b = Re(psi_b^H hpsi_b) / (psi_b^H psi_b)            (Algorithm 12 line 3)
+// lambda_b = Re(psi_b^H hpsi_b) / Re(psi_b^H spsi_b), spsi = S psi (null: S = I)      (Algorithm 12 line 3)
 __global__ void __launch_bounds__(RT) k_rayleigh(int64_t npw, const c128* __restrict__ psi, int64_t ld,
-                                                 const c128* __restrict__ hpsi, int64_t ldh, double* __restrict__ lambda,
-                                                 double* __restrict__ nrm2) {
+                                                 const c128* __restrict__ hpsi, int64_t ldh, const c128* __restrict__ spsi,
+                                                 int64_t lds, double* __restrict__ lambda, double* __restrict__ nrm2) {
   __shared__ double red[RT / 32];
   const c128* x = psi + (int64_t)blockIdx.x * ld;
   const c128* y = hpsi + (int64_t)blockIdx.x * ldh;
+  const c128* z = spsi ? spsi + (int64_t)blockIdx.x * lds : x;
   double num = 0.0, den = 0.0;
   for (int64_t g = threadIdx.x; g < npw; g += RT) {
-    const c128 a = x[g], b = y[g];
+    const c128 a = x[g], b = y[g], c = z[g];
     num = fma(a.x, b.x, fma(a.y, b.y, num));
-    den = fma(a.x, a.x, fma(a.y, a.y, den));
+    den = fma(a.x, c.x, fma(a.y, c.y, den));
   }
   num = block_sum(num, red);
   den = block_sum(den, red);
@@ -90,7 +91,8 @@ __global__ void __launch_bounds__(RT) k_minmax(int64_t n, const double* __restri
   }
 }
 
-// W_b = hpsi_b - lambda_b psi_b (stored when W != null), norms_b = ||W_b||_2      (Algorithm 12 lines 11-12, S = I)
+// W_b = hpsi_b - lambda_b spsi_b (stored when W != null), norms_b = ||W_b||_2; `psi` is S psi for the generalised problem
+// (Algorithm 12 lines 11-12: W <- (H - Lambda S) Psi)
 __global__ void __launch_bounds__(RT) k_residual(int64_t npw, const c128* __restrict__ psi, int64_t ld,
                                                  const c128* __restrict__ hpsi, int64_t ldh,
                                                  const double* __restrict__ lambda, c128* __restrict__ W, int64_t ldw,
@@ -367,11 +369,11 @@ void launch_merge_info(const int* potrf_info, int* info, cudaStream_t st) {
 // ---------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------
-void launch_rayleigh(int64_t npw, int64_t nband, const c128* psi, int64_t ld, const c128* hpsi, int64_t ldh, double* lambda,
-                     double* nrm2, double* minmax, cudaStream_t st) {
+void launch_rayleigh(int64_t npw, int64_t nband, const c128* psi, int64_t ld, const c128* hpsi, int64_t ldh,
+                     const c128* spsi, int64_t lds, double* lambda, double* nrm2, double* minmax, cudaStream_t st) {
   {
     ScopedLaunch sl(ST_COLSTATS, st);
-    k_rayleigh<<<(unsigned)nband, RT, 0, st>>>(npw, psi, ld, hpsi, ldh, lambda, nrm2);
+    k_rayleigh<<<(unsigned)nband, RT, 0, st>>>(npw, psi, ld, hpsi, ldh, spsi, lds, lambda, nrm2);
   }
   if (minmax) {
     ScopedLaunch sl(ST_SMALL, st);

@@ -158,19 +158,21 @@ int pwh_sweep_host(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi_hos
  */
 
 /*
- * pwh_rayleigh_quotients -- lambda[i] = Re(psi_i^H hpsi_i) / (psi_i^H psi_i)  ("Rayleigh quotients
+ * pwh_rayleigh_quotients -- lambda[i] = Re(psi_i^H hpsi_i) / Re(psi_i^H spsi_i)  ("Rayleigh quotients
  * lambda_i = (H psi_i)^T psi_i / ((S psi_i)^T psi_i)", Algorithm 12 line 3), and, when minmax != NULL, minmax[0] = min_i,
  * minmax[1] = max_i lambda[i] -- the interval the filter is built on.  lambda: nband doubles, minmax: 2 doubles.
+ * In this and the following calls `spsi` = S Psi of the generalised problem; spsi == NULL means S = I.
  */
 int pwh_rayleigh_quotients(int64_t npw, int64_t nband, const pwh_c128* psi, int64_t ld, const pwh_c128* hpsi, int64_t ldh,
-                           double* lambda, double* minmax, void* stream);
+                           const pwh_c128* spsi, int64_t lds, double* lambda, double* minmax, void* stream);
 
 /*
- * pwh_residual_norms -- W_i = hpsi_i - lambda[i] psi_i and norms[i] = ||W_i||_2  (Algorithm 12 lines 11-12 with S = I:
+ * pwh_residual_norms -- W_i = hpsi_i - lambda[i] spsi_i and norms[i] = ||W_i||_2  (Algorithm 12 lines 11-12:
  * "W <- (H - Lambda S) Psi; compute residual norms").  W may be NULL (norms only); W may not alias the inputs.
  */
 int pwh_residual_norms(int64_t npw, int64_t nband, const pwh_c128* psi, int64_t ld, const pwh_c128* hpsi, int64_t ldh,
-                       const double* lambda, pwh_c128* W, int64_t ldw, double* norms, void* stream);
+                       const pwh_c128* spsi, int64_t lds, const double* lambda, pwh_c128* W, int64_t ldw, double* norms,
+                       void* stream);
 
 /*
  * pwh_rotate -- Y = X Q: X npw x m (ldx), Q m x n column-major (ldq >= m), Y npw x n (ldy); Y must not overlap X
@@ -213,15 +215,16 @@ int pwh_chol_ortho(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c1
                    int64_t ldu, int32_t* info, void* ws, size_t ws_bytes, void* stream);
 
 /*
- * pwh_rayleigh_ritz -- Algorithm 10 (RR) with S = I, in place: H_Psi = Psi^H (H Psi), S_Psi = Psi^H Psi,
- * H_Psi X = S_Psi X Lambda, Psi <- Psi X, H Psi <- (H Psi) X (Algorithm 5).  lambda
- * receives the nband Ritz values in ascending order; afterwards Psi^H Psi = I and Psi^H (H Psi) = diag(lambda).
+ * pwh_rayleigh_ritz -- Algorithm 10 (RR), in place: H_Psi = Psi^H (H Psi), S_Psi = Psi^H (S Psi), H_Psi X = S_Psi X Lambda,
+ * Psi <- Psi X, H Psi <- (H Psi) X, S Psi <- (S Psi) X (Algorithm 5).  lambda receives
+ * the nband Ritz values in ascending order; afterwards Psi^H (S Psi) = I and Psi^H (H Psi) = diag(lambda).
  */
-int pwh_rayleigh_ritz(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh, double* lambda,
-                      int32_t* info, void* ws, size_t ws_bytes, void* stream);
+int pwh_rayleigh_ritz(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh, pwh_c128* spsi,
+                      int64_t lds, double* lambda, int32_t* info, void* ws, size_t ws_bytes, void* stream);
 
 /*
- * pwh_chebfi_iteration -- one iteration of Algorithm 12 with S = I, in place on psi:
+ * pwh_chebfi_iteration -- one iteration of Algorithm 12, in place on psi (spsi == NULL: S = I;
+ * otherwise the handle must carry PAW blocks, H Psi and S Psi come from pwh_apply_hs and the filter is pwh_cheb_filter_gen):
  *   H Psi (lines 1-2); Rayleigh quotients, a = max, a0 = min - a0_margin (line 3; reading R5: the upper bound b
  *   of the spectrum is an input); Psi <- p_degree(H) Psi in column blocks of `block` (lines 4-8); H Psi; Rayleigh-Ritz
  *   (line 10); residual norms of the Ritz pairs (lines 11-12).
@@ -232,8 +235,41 @@ int pwh_rayleigh_ritz(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh
  */
 size_t pwh_chebfi_workspace_bytes(const pwh_ham* ham, int64_t nband, int64_t block);
 int pwh_chebfi_iteration(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh,
-                         int degree, double b, double a0_margin, double* lambda, double* resid, double* bounds_host,
-                         int32_t* info, void* ws, size_t ws_bytes, void* stream);
+                         pwh_c128* spsi, int64_t lds, int degree, double b, double a0_margin, double* lambda, double* resid,
+                         double* bounds_host, int32_t* info, void* ws, size_t ws_bytes, void* stream);
+
+/*
+ * ---------------------------------------------------------------------------------------------------------------
+ * PAW-style generalised problem H Psi = Lambda S Psi ("S != I whenever the norm constraint is relaxed, as
+ * in the Projector Augmented-Wave approach"; every benchmark of the paper uses PAW).
+ *     V_nonloc = sum_{R,i,j} |p_i^R> D_ij^R <p_j^R|,     S = I + sum_{R,i,j} |p_i^R> Q_ij^R <p_j^R|
+ * ---------------------------------------------------------------------------------------------------------------
+ *
+ * pwh_ham_set_paw -- replaces the diagonal D of the handle by per-atom dense Hermitian blocks D^R and adds the overlap
+ * blocks Q^R.  The projector index is cut into `nblocks` consecutive blocks: offsets (HOST, nblocks + 1 int32, offsets[0] =
+ * 0, offsets[nblocks] = nproj); dblocks / qblocks (DEVICE) hold the blocks one after the other, each n_R x n_R
+ * column-major.  Both are copied.  The call also builds the nproj x nproj matrix K of S^-1 = I - P K P^H (Woodbury,
+ * PAPER.md:225, 252) with two Cholesky factorisations (G = P^H P and I + U Q U^H) on the device, allocates scratch for it,
+ * and synchronises the stream.  *info (DEVICE int32) = 0, or < 0 when one of the two matrices is not positive definite
+ * (linearly dependent projectors, or an overlap S that is not positive definite).  Afterwards pwh_apply_h,
+ * pwh_cheb_filter and the host entry points use the dense D^R; S enters through the calls below.
+ */
+int pwh_ham_set_paw(pwh_ham* ham, int64_t nblocks, const int32_t* offsets, const pwh_c128* dblocks, const pwh_c128* qblocks,
+                    int32_t* info, void* stream);
+
+/*
+ * pwh_apply_hs -- HX_SX: hpsi = H psi and spsi = S psi from ONE set of projections C = P^H psi
+ * (either output may be NULL).  Workspace as for pwh_apply_h; psi must not overlap the outputs.
+ * pwh_apply_sinv -- Sinv: x <- S^-1 x = x - P K (P^H x), in place.
+ * pwh_cheb_filter_gen -- the scaled Chebyshev filter of degree m of the operator S^-1 H, in place (Algorithm 12 lines 4-8,
+ * per degree one H application, one Sinv and the three-term axpy of PAPER.md:246); same recurrence,
+ * bounds and errors as pwh_cheb_filter.
+ */
+int pwh_apply_hs(pwh_ham* ham, int64_t nband, const pwh_c128* psi, int64_t ldpsi, pwh_c128* hpsi, int64_t ldh, pwh_c128* spsi,
+                 int64_t lds, void* ws, size_t ws_bytes, void* stream);
+int pwh_apply_sinv(pwh_ham* ham, int64_t nband, pwh_c128* x, int64_t ldx, void* ws, size_t ws_bytes, void* stream);
+int pwh_cheb_filter_gen(pwh_ham* ham, int64_t nband, pwh_c128* psi, int64_t ld, int degree, double a, double b, double a0,
+                        void* ws, size_t ws_bytes, void* stream);
 
 /* Number of kernel launches issued by this library since load (all handles, all threads). */
 int64_t pwh_launch_count(void);

@@ -26,7 +26,8 @@ EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply
            "pwh_probe_fp64_tensor_peak",
            "pwh_rayleigh_quotients", "pwh_residual_norms", "pwh_rotate", "pwh_dense_workspace_bytes", "pwh_potrf",
            "pwh_heev", "pwh_hegv", "pwh_rr_workspace_bytes", "pwh_chol_ortho", "pwh_rayleigh_ritz",
-           "pwh_chebfi_workspace_bytes", "pwh_chebfi_iteration"]
+           "pwh_chebfi_workspace_bytes", "pwh_chebfi_iteration",
+           "pwh_ham_set_paw", "pwh_apply_hs", "pwh_apply_sinv", "pwh_cheb_filter_gen"]
 
 STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "colstats", "dense_small",
           "jacobi", "axpy", "reserved10", "reserved11"]
@@ -84,9 +85,9 @@ def load_library() -> ctypes.CDLL:
     L.pwh_probe_fp64_tensor_peak.restype = i32
     L.pwh_last_error.argtypes = []
     L.pwh_last_error.restype = ctypes.c_char_p
-    L.pwh_rayleigh_quotients.argtypes = [i64, i64, vp, i64, vp, i64, vp, vp, vp]
+    L.pwh_rayleigh_quotients.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, vp, vp]
     L.pwh_rayleigh_quotients.restype = i32
-    L.pwh_residual_norms.argtypes = [i64, i64, vp, i64, vp, i64, vp, vp, i64, vp, vp]
+    L.pwh_residual_norms.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, vp, i64, vp, vp]
     L.pwh_residual_norms.restype = i32
     L.pwh_rotate.argtypes = [i64, i64, vp, i64, i64, vp, i64, vp, i64, vp]
     L.pwh_rotate.restype = i32
@@ -102,12 +103,20 @@ def load_library() -> ctypes.CDLL:
     L.pwh_rr_workspace_bytes.restype = sz
     L.pwh_chol_ortho.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, vp, sz, vp]
     L.pwh_chol_ortho.restype = i32
-    L.pwh_rayleigh_ritz.argtypes = [i64, i64, vp, i64, vp, i64, vp, vp, vp, sz, vp]
+    L.pwh_rayleigh_ritz.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, vp, vp, sz, vp]
     L.pwh_rayleigh_ritz.restype = i32
     L.pwh_chebfi_workspace_bytes.argtypes = [vp, i64, i64]
     L.pwh_chebfi_workspace_bytes.restype = sz
-    L.pwh_chebfi_iteration.argtypes = [vp, i64, i64, vp, i64, vp, i64, i32, dbl, dbl, vp, vp, vp, vp, vp, sz, vp]
+    L.pwh_chebfi_iteration.argtypes = [vp, i64, i64, vp, i64, vp, i64, vp, i64, i32, dbl, dbl, vp, vp, vp, vp, vp, sz, vp]
     L.pwh_chebfi_iteration.restype = i32
+    L.pwh_ham_set_paw.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+    L.pwh_ham_set_paw.restype = i32
+    L.pwh_apply_hs.argtypes = [vp, i64, vp, i64, vp, i64, vp, i64, vp, sz, vp]
+    L.pwh_apply_hs.restype = i32
+    L.pwh_apply_sinv.argtypes = [vp, i64, vp, i64, vp, sz, vp]
+    L.pwh_apply_sinv.restype = i32
+    L.pwh_cheb_filter_gen.argtypes = [vp, i64, vp, i64, i32, dbl, dbl, dbl, vp, sz, vp]
+    L.pwh_cheb_filter_gen.restype = i32
     _lib = L
     return L
 
@@ -359,33 +368,40 @@ def _cm(a: torch.Tensor) -> torch.Tensor:
     return a.to(torch.complex128).T.contiguous().clone()
 
 
-def rayleigh_quotients(psi: torch.Tensor, hpsi: torch.Tensor):
-    """pwh_rayleigh_quotients: (lambda (nband,), minmax (2,)) as device tensors."""
+def _opt_block(t: Optional[torch.Tensor], npw: int, name: str):
+    return (None, npw) if t is None else _block_args(t, npw, name)
+
+
+def rayleigh_quotients(psi: torch.Tensor, hpsi: torch.Tensor, spsi: Optional[torch.Tensor] = None):
+    """pwh_rayleigh_quotients: (lambda (nband,), minmax (2,)) as device tensors; spsi = S psi (None: S = I)."""
     L = load_library()
     npw = int(psi.shape[1])
     p, ld = _block_args(psi, npw, "psi")
     h, ldh = _block_args(hpsi, npw, "hpsi")
+    s_, lds = _opt_block(spsi, npw, "spsi")
     nb = int(psi.shape[0])
     lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
     mm = torch.empty(2, dtype=torch.float64, device=psi.device)
     with torch.cuda.device(psi.device):
-        _check(L.pwh_rayleigh_quotients(npw, nb, p, ld, h, ldh, lam.data_ptr(), mm.data_ptr(), _stream_ptr(psi.device)),
-               "pwh_rayleigh_quotients")
+        _check(L.pwh_rayleigh_quotients(npw, nb, p, ld, h, ldh, s_, lds, lam.data_ptr(), mm.data_ptr(),
+                                        _stream_ptr(psi.device)), "pwh_rayleigh_quotients")
     return lam, mm
 
 
-def residual_norms(psi: torch.Tensor, hpsi: torch.Tensor, lam: torch.Tensor, want_w: bool = False):
-    """pwh_residual_norms: norms (nband,) and, when want_w, W = hpsi - lam psi."""
+def residual_norms(psi: torch.Tensor, hpsi: torch.Tensor, lam: torch.Tensor, want_w: bool = False,
+                   spsi: Optional[torch.Tensor] = None):
+    """pwh_residual_norms: norms (nband,) and, when want_w, W = hpsi - lam spsi (spsi None: psi)."""
     L = load_library()
     npw = int(psi.shape[1])
     p, ld = _block_args(psi, npw, "psi")
     h, ldh = _block_args(hpsi, npw, "hpsi")
+    s_, lds = _opt_block(spsi, npw, "spsi")
     nb = int(psi.shape[0])
     lam = lam.to(device=psi.device, dtype=torch.float64).contiguous()
     norms = torch.empty(nb, dtype=torch.float64, device=psi.device)
     w = torch.empty_like(psi) if want_w else None
     with torch.cuda.device(psi.device):
-        _check(L.pwh_residual_norms(npw, nb, p, ld, h, ldh, lam.data_ptr(), w.data_ptr() if want_w else None, npw,
+        _check(L.pwh_residual_norms(npw, nb, p, ld, h, ldh, s_, lds, lam.data_ptr(), w.data_ptr() if want_w else None, npw,
                                     norms.data_ptr(), _stream_ptr(psi.device)), "pwh_residual_norms")
     return (norms, w) if want_w else norms
 
@@ -460,28 +476,31 @@ def chol_ortho(psi: torch.Tensor, hpsi: Optional[torch.Tensor] = None):
     return u.T, int(info.item())
 
 
-def rayleigh_ritz(psi: torch.Tensor, hpsi: torch.Tensor):
-    """pwh_rayleigh_ritz, in place on psi and hpsi: returns (lambda (nband,), info)."""
+def rayleigh_ritz(psi: torch.Tensor, hpsi: torch.Tensor, spsi: Optional[torch.Tensor] = None):
+    """pwh_rayleigh_ritz, in place on psi, hpsi (and spsi): returns (lambda (nband,), info)."""
     L = load_library()
     npw = int(psi.shape[1])
     p, ld = _block_args(psi, npw, "psi")
     h, ldh = _block_args(hpsi, npw, "hpsi")
+    s_, lds = _opt_block(spsi, npw, "spsi")
     nb = int(psi.shape[0])
     lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
     info = torch.zeros(1, dtype=torch.int32, device=psi.device)
     ws = _ws(psi.device, int(L.pwh_rr_workspace_bytes(npw, nb)))
     with torch.cuda.device(psi.device):
-        _check(L.pwh_rayleigh_ritz(npw, nb, p, ld, h, ldh, lam.data_ptr(), info.data_ptr(), ws.data_ptr(), ws.numel(),
+        _check(L.pwh_rayleigh_ritz(npw, nb, p, ld, h, ldh, s_, lds, lam.data_ptr(), info.data_ptr(), ws.data_ptr(), ws.numel(),
                                    _stream_ptr(psi.device)), "pwh_rayleigh_ritz")
     return lam, int(info.item())
 
 
 def chebfi_iteration(ham: Ham, psi: torch.Tensor, hpsi: torch.Tensor, degree: int, b: float, a0_margin: float = 0.0,
-                     block: int = 0):
-    """pwh_chebfi_iteration, in place on psi / hpsi: returns dict(lam, resid (device tensors), a0, a, info)."""
+                     block: int = 0, spsi: Optional[torch.Tensor] = None):
+    """pwh_chebfi_iteration, in place on psi / hpsi (/ spsi: generalised problem, needs set_paw): returns
+    dict(lam, resid (device tensors), a0, a, info)."""
     L = load_library()
     p, ld = _block_args(psi, ham.npw, "psi")
     h, ldh = _block_args(hpsi, ham.npw, "hpsi")
+    s_, lds = _opt_block(spsi, ham.npw, "spsi")
     nb = int(psi.shape[0])
     lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
     res = torch.empty(nb, dtype=torch.float64, device=psi.device)
@@ -489,10 +508,67 @@ def chebfi_iteration(ham: Ham, psi: torch.Tensor, hpsi: torch.Tensor, degree: in
     bounds = (ctypes.c_double * 2)()
     ws = _ws(psi.device, int(L.pwh_chebfi_workspace_bytes(ham.handle, nb, int(block))), tag="chebfi")
     with torch.cuda.device(ham.device):
-        _check(L.pwh_chebfi_iteration(ham.handle, nb, int(block), p, ld, h, ldh, int(degree), float(b), float(a0_margin),
+        _check(L.pwh_chebfi_iteration(ham.handle, nb, int(block), p, ld, h, ldh, s_, lds, int(degree), float(b), float(a0_margin),
                                       lam.data_ptr(), res.data_ptr(), bounds, info.data_ptr(), ws.data_ptr(), ws.numel(),
                                       _stream_ptr(ham.device)), "pwh_chebfi_iteration")
     return {"lam": lam, "resid": res, "a0": float(bounds[0]), "a": float(bounds[1]), "info": int(info.item())}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# PAW-style generalised problem
+# ----------------------------------------------------------------------------------------------------------------
+def ham_set_paw(ham: Ham, offsets, dblocks, qblocks) -> int:
+    """pwh_ham_set_paw: per-atom dense blocks D^R, Q^R (lists of (n_R, n_R) arrays indexed [i, j]); returns info."""
+    L = load_library()
+    offsets = np.ascontiguousarray(np.asarray(offsets, dtype=np.int32))
+
+    def pack(blocks):
+        flat = np.concatenate([np.asarray(b, dtype=np.complex128).T.reshape(-1) for b in blocks])   # column-major
+        return torch.from_numpy(np.ascontiguousarray(flat)).to(ham.device)
+
+    d, q = pack(dblocks), pack(qblocks)
+    info = torch.zeros(1, dtype=torch.int32, device=ham.device)
+    with torch.cuda.device(ham.device):
+        _check(L.pwh_ham_set_paw(ham.handle, len(offsets) - 1, offsets.ctypes.data, d.data_ptr(), q.data_ptr(),
+                                 info.data_ptr(), _stream_ptr(ham.device)), "pwh_ham_set_paw")
+    ham._ws = None                     # the workspace layout grows with the PAW blocks
+    return int(info.item())
+
+
+def apply_hs(ham: Ham, psi: torch.Tensor):
+    """pwh_apply_hs: returns (H psi, S psi)."""
+    L = load_library()
+    p, ldp = _block_args(psi, ham.npw, "psi")
+    nband = int(psi.shape[0])
+    hpsi, spsi = torch.empty_like(psi), torch.empty_like(psi)
+    ws = ham.workspace(nband)
+    with torch.cuda.device(ham.device):
+        _check(L.pwh_apply_hs(ham.handle, nband, p, ldp, hpsi.data_ptr(), ham.npw, spsi.data_ptr(), ham.npw, ws.data_ptr(),
+                              ws.numel(), _stream_ptr(ham.device)), "pwh_apply_hs")
+    return hpsi, spsi
+
+
+def apply_sinv(ham: Ham, x: torch.Tensor) -> torch.Tensor:
+    """pwh_apply_sinv: x <- S^-1 x in place; returns x."""
+    L = load_library()
+    p, ld = _block_args(x, ham.npw, "x")
+    nband = int(x.shape[0])
+    ws = ham.workspace(nband)
+    with torch.cuda.device(ham.device):
+        _check(L.pwh_apply_sinv(ham.handle, nband, p, ld, ws.data_ptr(), ws.numel(), _stream_ptr(ham.device)), "pwh_apply_sinv")
+    return x
+
+
+def cheb_filter_gen(ham: Ham, psi: torch.Tensor, degree: int, a: float, b: float, a0: float) -> torch.Tensor:
+    """pwh_cheb_filter_gen: in place psi <- p_m(S^-1 H) psi; returns psi."""
+    L = load_library()
+    p, ld = _block_args(psi, ham.npw, "psi")
+    nband = int(psi.shape[0])
+    ws = ham.workspace(nband)
+    with torch.cuda.device(ham.device):
+        _check(L.pwh_cheb_filter_gen(ham.handle, nband, p, ld, int(degree), float(a), float(b), float(a0), ws.data_ptr(),
+                                     ws.numel(), _stream_ptr(ham.device)), "pwh_cheb_filter_gen")
+    return psi
 
 
 def launch_count() -> int:

@@ -52,26 +52,33 @@ static int check_ws(const void* ws, size_t have, size_t need) {
 }
 
 extern "C" int pwh_rayleigh_quotients(int64_t npw, int64_t nband, const pwh_c128* psi, int64_t ld, const pwh_c128* hpsi,
-                                      int64_t ldh, double* lambda, double* minmax, void* stream) {
+                                      int64_t ldh, const pwh_c128* spsi, int64_t lds, double* lambda, double* minmax,
+                                      void* stream) {
   if (npw < 1 || nband < 0) return api_fail(PWH_EINVAL, "bad sizes");
   if (nband == 0) return PWH_OK;
   int rc;
   if ((rc = check_block(psi, ld, npw, "psi")) || (rc = check_block(hpsi, ldh, npw, "hpsi"))) return rc;
+  if (spsi && lds < npw) return api_fail(PWH_EINVAL, "spsi: leading dimension smaller than npw");
   if (!lambda) return api_fail(PWH_EINVAL, "lambda is null");
-  launch_rayleigh(npw, nband, (const c128*)psi, ld, (const c128*)hpsi, ldh, lambda, nullptr, minmax, (cudaStream_t)stream);
+  launch_rayleigh(npw, nband, (const c128*)psi, ld, (const c128*)hpsi, ldh, (const c128*)spsi, lds, lambda, nullptr, minmax,
+                  (cudaStream_t)stream);
   RR_TRY(cudaGetLastError());
   return PWH_OK;
 }
 
 extern "C" int pwh_residual_norms(int64_t npw, int64_t nband, const pwh_c128* psi, int64_t ld, const pwh_c128* hpsi,
-                                  int64_t ldh, const double* lambda, pwh_c128* W, int64_t ldw, double* norms, void* stream) {
+                                  int64_t ldh, const pwh_c128* spsi, int64_t lds, const double* lambda, pwh_c128* W,
+                                  int64_t ldw, double* norms, void* stream) {
   if (npw < 1 || nband < 0) return api_fail(PWH_EINVAL, "bad sizes");
   if (nband == 0) return PWH_OK;
   int rc;
   if ((rc = check_block(psi, ld, npw, "psi")) || (rc = check_block(hpsi, ldh, npw, "hpsi"))) return rc;
+  if (spsi && lds < npw) return api_fail(PWH_EINVAL, "spsi: leading dimension smaller than npw");
   if (W && ldw < npw) return api_fail(PWH_EINVAL, "W: leading dimension smaller than npw");
   if (!lambda || !norms) return api_fail(PWH_EINVAL, "lambda / norms null");
-  launch_residual(npw, nband, (const c128*)psi, ld, (const c128*)hpsi, ldh, lambda, (c128*)W, ldw, norms, (cudaStream_t)stream);
+  // W = H psi - lambda S psi: the kernel's "psi" operand is S psi for the generalised problem
+  launch_residual(npw, nband, spsi ? (const c128*)spsi : (const c128*)psi, spsi ? lds : ld, (const c128*)hpsi, ldh, lambda,
+                  (c128*)W, ldw, norms, (cudaStream_t)stream);
   RR_TRY(cudaGetLastError());
   return PWH_OK;
 }
@@ -233,11 +240,13 @@ extern "C" int pwh_chol_ortho(int64_t npw, int64_t nband, pwh_c128* psi, int64_t
 }
 
 extern "C" int pwh_rayleigh_ritz(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh,
-                                 double* lambda, int32_t* info, void* ws, size_t ws_bytes, void* stream) {
+                                 pwh_c128* spsi, int64_t lds, double* lambda, int32_t* info, void* ws, size_t ws_bytes,
+                                 void* stream) {
   if (npw < 1 || nband < 0) return api_fail(PWH_EINVAL, "bad sizes");
   if (nband == 0) return PWH_OK;
   int rc;
   if ((rc = check_block(psi, ld, npw, "psi")) || (rc = check_block(hpsi, ldh, npw, "hpsi"))) return rc;
+  if (spsi && lds < npw) return api_fail(PWH_EINVAL, "spsi: leading dimension smaller than npw");
   if (!lambda || !info) return api_fail(PWH_EINVAL, "lambda / info null");
   const RrWs r = rr_layout(npw, nband);
   if ((rc = check_ws(ws, ws_bytes, r.total))) return rc;
@@ -246,16 +255,19 @@ extern "C" int pwh_rayleigh_ritz(int64_t npw, int64_t nband, pwh_c128* psi, int6
   c128* Hs = (c128*)(wsb + r.hs);
   c128* Ss = (c128*)(wsb + r.ss);
   c128* X = (c128*)(wsb + r.x);
-  // H_Psi = Psi^H (H Psi), S_Psi = Psi^H Psi  (Algorithm 10 steps 1-2), both Hermitian
+  // H_Psi = Psi^H (H Psi), S_Psi = Psi^H (S Psi)  (Algorithm 10 steps 1-2), both Hermitian
   if ((rc = pwh_gram_herm(npw, nband, psi, ld, hpsi, ldh, (pwh_c128*)Hs, nband, wsb + r.gram, r.total - r.gram, stream))) return rc;
-  if ((rc = pwh_gram_herm(npw, nband, psi, ld, psi, ld, (pwh_c128*)Ss, nband, wsb + r.gram, r.total - r.gram, stream))) return rc;
+  if ((rc = pwh_gram_herm(npw, nband, psi, ld, spsi ? spsi : psi, spsi ? lds : ld, (pwh_c128*)Ss, nband, wsb + r.gram,
+                          r.total - r.gram, stream))) return rc;
   launch_hermitise((int)nband, Hs, nband, st);
   launch_hermitise((int)nband, Ss, nband, st);
   // H_Psi X = S_Psi X Lambda  (step 3)
   if ((rc = hegv_impl(nband, Hs, nband, Ss, nband, lambda, X, nband, info, wsb + r.dense, r.d, st))) return rc;
-  // Psi <- Psi X, H Psi <- (H Psi) X  (steps 4-5)
+  // Psi <- Psi X, H Psi <- (H Psi) X, S Psi <- (S Psi) X  (steps 4-6)
   if ((rc = rotate_inplace(npw, nband, (c128*)psi, ld, X, nband, (c128*)(wsb + r.panel), st))) return rc;
-  return rotate_inplace(npw, nband, (c128*)hpsi, ldh, X, nband, (c128*)(wsb + r.panel), st);
+  if ((rc = rotate_inplace(npw, nband, (c128*)hpsi, ldh, X, nband, (c128*)(wsb + r.panel), st))) return rc;
+  if (spsi && (rc = rotate_inplace(npw, nband, (c128*)spsi, lds, X, nband, (c128*)(wsb + r.panel), st))) return rc;
+  return PWH_OK;
 }
 
 extern "C" size_t pwh_chebfi_workspace_bytes(const pwh_ham* ham, int64_t nband, int64_t block) {
@@ -266,8 +278,9 @@ extern "C" size_t pwh_chebfi_workspace_bytes(const pwh_ham* ham, int64_t nband, 
 }
 
 extern "C" int pwh_chebfi_iteration(pwh_ham* ham, int64_t nband, int64_t block, pwh_c128* psi, int64_t ld, pwh_c128* hpsi,
-                                    int64_t ldh, int degree, double b, double a0_margin, double* lambda, double* resid,
-                                    double* bounds_host, int32_t* info, void* ws, size_t ws_bytes, void* stream) {
+                                    int64_t ldh, pwh_c128* spsi, int64_t lds, int degree, double b, double a0_margin,
+                                    double* lambda, double* resid, double* bounds_host, int32_t* info, void* ws,
+                                    size_t ws_bytes, void* stream) {
   int64_t hi[8];
   if (!ham || pwh_ham_info(ham, hi) != PWH_OK) return api_fail(PWH_EINVAL, "handle is null");
   const int64_t npw = hi[0];
@@ -276,6 +289,7 @@ extern "C" int pwh_chebfi_iteration(pwh_ham* ham, int64_t nband, int64_t block, 
   if (!(a0_margin >= 0.0)) return api_fail(PWH_EINVAL, "a0_margin < 0");
   int rc;
   if ((rc = check_block(psi, ld, npw, "psi")) || (rc = check_block(hpsi, ldh, npw, "hpsi"))) return rc;
+  if (spsi && lds < npw) return api_fail(PWH_EINVAL, "spsi: leading dimension smaller than npw");
   if (!lambda || !resid || !info) return api_fail(PWH_EINVAL, "lambda / resid / info null");
   if (block <= 0 || block > nband) block = nband;
   const size_t need = pwh_chebfi_workspace_bytes(ham, nband, block);
@@ -283,13 +297,20 @@ extern "C" int pwh_chebfi_iteration(pwh_ham* ham, int64_t nband, int64_t block, 
   cudaStream_t st = (cudaStream_t)stream;
   unsigned char* wsb = (unsigned char*)ws;
   double* d_minmax = (double*)(wsb + need - 256);
-  // lines 1-2: H Psi
-  for (int64_t b0 = 0; b0 < nband; b0 += block) {
-    const int64_t nb = std::min(block, nband - b0);
-    if ((rc = pwh_apply_h(ham, nb, psi + b0 * ld, ld, hpsi + b0 * ldh, ldh, ws, need - 256, stream))) return rc;
-  }
+  // H Psi (and S Psi: HX_SX) in column blocks
+  auto hx_sx = [&]() -> int {
+    for (int64_t b0 = 0; b0 < nband; b0 += block) {
+      const int64_t nb = std::min(block, nband - b0);
+      const int r = spsi ? pwh_apply_hs(ham, nb, psi + b0 * ld, ld, hpsi + b0 * ldh, ldh, spsi + b0 * lds, lds, ws, need - 256, stream)
+                         : pwh_apply_h(ham, nb, psi + b0 * ld, ld, hpsi + b0 * ldh, ldh, ws, need - 256, stream);
+      if (r) return r;
+    }
+    return PWH_OK;
+  };
+  // lines 1-2
+  if ((rc = hx_sx())) return rc;
   // line 3: Rayleigh quotients, their minimum and maximum -> the filter's interval (the one host round trip of the iteration)
-  launch_rayleigh(npw, nband, (const c128*)psi, ld, (const c128*)hpsi, ldh, lambda, nullptr, d_minmax, st);
+  launch_rayleigh(npw, nband, (const c128*)psi, ld, (const c128*)hpsi, ldh, (const c128*)spsi, lds, lambda, nullptr, d_minmax, st);
   double mm[2];
   RR_TRY(cudaMemcpyAsync(mm, d_minmax, sizeof(mm), cudaMemcpyDeviceToHost, st));
   RR_TRY(cudaStreamSynchronize(st));
@@ -297,18 +318,18 @@ extern "C" int pwh_chebfi_iteration(pwh_ham* ham, int64_t nband, int64_t block, 
   if (bounds_host) { bounds_host[0] = a0; bounds_host[1] = a; }
   if (!(b > a) || !(a0 < a))
     return api_fail(PWH_EINVAL, "Rayleigh quotients span [%g, %g]: need min - a0_margin < max < b = %g", mm[0], mm[1], b);
-  // lines 4-8: the filter
+  // lines 4-8: the filter (of S^-1 H when the overlap is not the identity)
   for (int64_t b0 = 0; b0 < nband; b0 += block) {
     const int64_t nb = std::min(block, nband - b0);
-    if ((rc = pwh_cheb_filter(ham, nb, psi + b0 * ld, ld, degree, a, b, a0, ws, need - 256, stream))) return rc;
+    rc = spsi ? pwh_cheb_filter_gen(ham, nb, psi + b0 * ld, ld, degree, a, b, a0, ws, need - 256, stream)
+              : pwh_cheb_filter(ham, nb, psi + b0 * ld, ld, degree, a, b, a0, ws, need - 256, stream);
+    if (rc) return rc;
   }
-  for (int64_t b0 = 0; b0 < nband; b0 += block) {
-    const int64_t nb = std::min(block, nband - b0);
-    if ((rc = pwh_apply_h(ham, nb, psi + b0 * ld, ld, hpsi + b0 * ldh, ldh, ws, need - 256, stream))) return rc;
-  }
+  if ((rc = hx_sx())) return rc;
   // line 10: Rayleigh-Ritz; lines 11-12: residuals
-  if ((rc = pwh_rayleigh_ritz(npw, nband, psi, ld, hpsi, ldh, lambda, info, ws, need - 256, stream))) return rc;
-  launch_residual(npw, nband, (const c128*)psi, ld, (const c128*)hpsi, ldh, lambda, nullptr, 0, resid, st);
+  if ((rc = pwh_rayleigh_ritz(npw, nband, psi, ld, hpsi, ldh, spsi, lds, lambda, info, ws, need - 256, stream))) return rc;
+  launch_residual(npw, nband, spsi ? (const c128*)spsi : (const c128*)psi, spsi ? lds : ld, (const c128*)hpsi, ldh, lambda,
+                  nullptr, 0, resid, st);
   RR_TRY(cudaGetLastError());
   return PWH_OK;
 }

@@ -232,11 +232,12 @@ def test_chebfi_iteration(gpu, cfg, degree, request):
     import torch
     w = request.getfixturevalue(cfg)
     ham = gpu.ham_setup(*ham_args(w))
-    psi = dev(w.psi)
+    nb = min(40, w.psi.shape[0])                  # the oracle filters at ~25 band-applications/s on cfg 2
+    psi = dev(w.psi[:nb])
     hpsi = torch.empty_like(psi)
-    psi_ref = w.psi
+    psi_ref = np.ascontiguousarray(w.psi[:nb])
     for it in range(2):
-        out = gpu.chebfi_iteration(ham, psi, hpsi, degree, w.b, a0_margin=0.01, block=64)
+        out = gpu.chebfi_iteration(ham, psi, hpsi, degree, w.b, a0_margin=0.01, block=24)
         ref = rr.chebfi_iteration(*ham_args(w), psi_ref, degree, w.b, a0_margin=0.01)
         assert out["info"] > 0
         assert out["a"] == pytest.approx(ref["a"], rel=1e-12) and out["a0"] == pytest.approx(ref["a0"], rel=1e-12)

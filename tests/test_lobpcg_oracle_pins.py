@@ -1,0 +1,82 @@
+"""Pins of the LOBPCG oracle (oracle/lobpcg_oracle.py, Algorithm 11 of the paper): hand values of the
+preconditioner, projector properties of S-Deflate, the nline = 0 special case (= Rayleigh-Ritz of the input, separately
+pinned), convergence to the dense spectrum (numpy.linalg.eigvalsh of oracle.dense_h) with Ritz values bounding it from
+above, fixed points (an exact invariant subspace stays put).  CPU only."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import lobpcg_oracle as lo
+from oracle import rr
+from paper_2604_11139_b200 import synth
+
+
+def ham_args(w):
+    return (w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, w.proj, w.dij)
+
+
+def test_tpa_preconditioner_hand_values():
+    kin = np.array([0.0, 1.0, 2.0, 1e6])
+    k = lo.tpa_preconditioner(kin, np.array([1.0, 2.0]))
+    assert k[0, 0] == 1.0                                               # x = 0
+    assert k[0, 1] == pytest.approx(65.0 / 81.0, rel=1e-15)             # x = 1: (27+18+12+8) / (65 + 16)
+    assert k[1, 2] == pytest.approx(65.0 / 81.0, rel=1e-15)             # x = kin / ekin = 2 / 2
+    assert k[0, 3] * 2e6 == pytest.approx(1.0, rel=1e-5)                # x -> infinity: K -> 1 / (2 x)
+    assert np.all(np.diff(lo.tpa_preconditioner(np.linspace(0, 50, 200), np.array([1.0]))[0]) < 0)   # decreasing in x
+
+
+def test_band_kinetic_and_deflate(cfg1):
+    w = cfg1
+    kin = oracle.kinetic(w.lattice, w.kpt, w.gvec)
+    e = np.zeros((2, w.npw), dtype=np.complex128)
+    e[0, 7] = 3.0j
+    e[1, 7], e[1, 100] = 1.0, 1.0
+    ek = lo.band_kinetic(kin, e)
+    assert ek[0] == pytest.approx(kin[7]) and ek[1] == pytest.approx(0.5 * (kin[7] + kin[100]))
+    basis = w.psi[:5]                                                   # orthonormal (cfg 1's block is)
+    x = w.psi[5:9] + 0.3 * w.psi[:4]
+    y = lo.deflate(x, basis)
+    assert np.abs(oracle.gram(basis, y)).max() <= 1e-14                 # orthogonal to the basis afterwards
+    assert np.abs(lo.deflate(y, basis) - y).max() <= 1e-14              # idempotent
+    assert np.abs(y - w.psi[5:9]).max() <= 1e-13                        # the admixture is removed exactly
+    assert lo.deflate(x, basis[:0]) is x
+
+
+def test_nline_zero_is_rayleigh_ritz_of_the_input(cfg1):
+    w = cfg1
+    out = lo.lobpcg(*ham_args(w), w.psi, 1, 0)
+    hpsi = oracle.apply_h(*ham_args(w), w.psi)
+    lam_ref = np.linalg.eigvalsh(oracle.gram(w.psi, hpsi))              # psi is orthonormal: standard problem (library)
+    assert np.abs(out["lam"] - lam_ref).max() <= 1e-12 * np.abs(lam_ref).max()
+    assert np.abs(out["psi"] @ out["psi"].conj().T - np.eye(w.psi.shape[0])).max() <= 1e-12
+
+
+@pytest.mark.parametrize("nblocks", [1, 2, 4])
+def test_converges_to_the_dense_spectrum(cfg1, nblocks):
+    w = cfg1
+    ev = np.linalg.eigvalsh(oracle.dense_h(*ham_args(w)))
+    M = w.psi.shape[0]
+    out = lo.lobpcg(*ham_args(w), w.psi, nblocks, 12)
+    lam = out["lam"]
+    assert np.all(np.diff(lam) >= -1e-12)
+    assert np.all(lam >= ev[:M] - 1e-9)                                 # Ritz values bound the spectrum from above
+    assert np.abs(lam[: M // 2] - ev[: M // 2]).max() < 1e-5
+    assert np.abs(out["psi"] @ out["psi"].conj().T - np.eye(M)).max() <= 1e-10
+    assert np.abs(out["hpsi"] - oracle.apply_h(*ham_args(w), out["psi"])).max() <= 1e-9
+    for hist in out["history"]:                                         # residuals of a block shrink along the line minimisations
+        assert hist[-1].max() < 0.1 * hist[0].max()
+    # more line minimisations never raise a Ritz value (the search space contains the previous iterate)
+    fewer = lo.lobpcg(*ham_args(w), w.psi, nblocks, 4)["lam"]
+    if nblocks == 1:
+        assert np.all(lam <= fewer + 1e-10)
+
+
+def test_exact_invariant_subspace_is_a_fixed_point(cfg1):
+    w = cfg1
+    ev, vec = np.linalg.eigh(oracle.dense_h(*ham_args(w)))
+    psi = np.ascontiguousarray(vec[:, :6].T)
+    out = lo.lobpcg(*ham_args(w), psi, 1, 2)
+    assert np.abs(out["lam"] - ev[:6]).max() <= 1e-10 * np.abs(ev).max()
+    assert out["resid"].max() <= 1e-8
+    p_ref = vec[:, :6] @ vec[:, :6].conj().T
+    assert np.abs(out["psi"].T @ out["psi"].conj() - p_ref).max() <= 1e-8

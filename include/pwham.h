@@ -271,6 +271,36 @@ int pwh_apply_sinv(pwh_ham* ham, int64_t nband, pwh_c128* x, int64_t ldx, void* 
 int pwh_cheb_filter_gen(pwh_ham* ham, int64_t nband, pwh_c128* psi, int64_t ld, int degree, double a, double b, double a0,
                         void* ws, size_t ws_bytes, void* stream);
 
+/*
+ * ---------------------------------------------------------------------------------------------------------------
+ * LOBPCG -- the paper's other iterative eigensolver, on the same H application (Algorithm 6;
+ * PAPER.md:506-574 Algorithm 11, here with S = I).  The paper's arithmetic-intensity argument (the filter
+ * applies H k+1 times per data movement, LOBPCG once) is measured with it.
+ * ---------------------------------------------------------------------------------------------------------------
+ *
+ * pwh_lobpcg -- Algorithm 11, in place on psi: the nband bands are cut into `nblocks` consecutive blocks of m = nband /
+ * nblocks bands (nband % nblocks == 0, 3 m <= npw); per block: S-Deflate against the blocks already solved (Algorithm 8, line
+ * 3), H Psi_i (line 6), S-Ortho (Algorithm 9, line 8), RR (Algorithm 10, line 9), then `nline` line minimisations (lines
+ * 10-28): residual W = (H - Lambda) Psi_i and its norms (lines 11-12), W <- K W with the diagonal Teter-Payne-Allan
+ * preconditioner K(G) = t / (t + 16 x^4), t = 27 + 18 x + 12 x^2 + 8 x^3, x = kin(G) / <T>_band (line 13; the paper names K
+ * "diagonal matrix" only, PAPER.md:504 -- DESIGN.md reading R16), S-Deflate (line 15), H W (line 18), S-Ortho and RR of
+ * [Psi_i, W_i] (first pass) or [Psi_i, W_i, P_i] (lines 20-25), whose lowest m Ritz pairs are the new Psi_i and whose part
+ * outside span(Psi_i) is the new P_i (line 26).  With nblocks > 1 a final S-Ortho + RR over all bands (lines 31-34).
+ *   tol       > 0: a block leaves the loop once all its residual norms are <= tol (line 12; costs one stream
+ *             synchronisation per line minimisation -- the paper's mpi-sR sits there); 0: always nline passes, no host sync.
+ *   lambda    [out] DEVICE nband Ritz values, ascending;  resid [out] DEVICE nband final residual norms (line 29);
+ *   history   [out, optional] DEVICE nblocks x nline x m doubles: the residual norms seen at line 12 (untouched entries for
+ *             passes skipped by the early exit);
+ *   info      [out] DEVICE int32: > 0 = largest Jacobi sweep count of the dense eigen-solves, < 0 = a Cholesky factorisation met
+ *             a non-positive pivot (linearly dependent search directions).
+ * hpsi receives H psi.  Workspace: pwh_lobpcg_workspace_bytes(ham, nband, nblocks) (0 for invalid arguments), 256-byte aligned.
+ * Errors: PWH_EINVAL for null pointers, bad sizes, ld < npw, workspace too small.
+ */
+size_t pwh_lobpcg_workspace_bytes(const pwh_ham* ham, int64_t nband, int64_t nblocks);
+int pwh_lobpcg(pwh_ham* ham, int64_t nband, int64_t nblocks, int nline, double tol, pwh_c128* psi, int64_t ld, pwh_c128* hpsi,
+               int64_t ldh, double* lambda, double* resid, double* history, int32_t* info, void* ws, size_t ws_bytes,
+               void* stream);
+
 /* Number of kernel launches issued by this library since load (all handles, all threads). */
 int64_t pwh_launch_count(void);
 

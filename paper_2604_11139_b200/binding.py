@@ -27,7 +27,8 @@ EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply
            "pwh_rayleigh_quotients", "pwh_residual_norms", "pwh_rotate", "pwh_dense_workspace_bytes", "pwh_potrf",
            "pwh_heev", "pwh_hegv", "pwh_rr_workspace_bytes", "pwh_chol_ortho", "pwh_rayleigh_ritz",
            "pwh_chebfi_workspace_bytes", "pwh_chebfi_iteration",
-           "pwh_ham_set_paw", "pwh_apply_hs", "pwh_apply_sinv", "pwh_cheb_filter_gen"]
+           "pwh_ham_set_paw", "pwh_apply_hs", "pwh_apply_sinv", "pwh_cheb_filter_gen",
+           "pwh_lobpcg_workspace_bytes", "pwh_lobpcg"]
 
 STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "colstats", "dense_small",
           "jacobi", "axpy", "reserved10", "reserved11"]
@@ -117,6 +118,10 @@ def load_library() -> ctypes.CDLL:
     L.pwh_apply_sinv.restype = i32
     L.pwh_cheb_filter_gen.argtypes = [vp, i64, vp, i64, i32, dbl, dbl, dbl, vp, sz, vp]
     L.pwh_cheb_filter_gen.restype = i32
+    L.pwh_lobpcg_workspace_bytes.argtypes = [vp, i64, i64]
+    L.pwh_lobpcg_workspace_bytes.restype = sz
+    L.pwh_lobpcg.argtypes = [vp, i64, i64, i32, dbl, vp, i64, vp, i64, vp, vp, vp, vp, vp, sz, vp]
+    L.pwh_lobpcg.restype = i32
     _lib = L
     return L
 
@@ -512,6 +517,28 @@ def chebfi_iteration(ham: Ham, psi: torch.Tensor, hpsi: torch.Tensor, degree: in
                                       lam.data_ptr(), res.data_ptr(), bounds, info.data_ptr(), ws.data_ptr(), ws.numel(),
                                       _stream_ptr(ham.device)), "pwh_chebfi_iteration")
     return {"lam": lam, "resid": res, "a0": float(bounds[0]), "a": float(bounds[1]), "info": int(info.item())}
+
+
+def lobpcg(ham: Ham, psi: torch.Tensor, hpsi: torch.Tensor, nblocks: int, nline: int, tol: float = 0.0):
+    """pwh_lobpcg (Algorithm 11, S = I), in place on psi / hpsi: returns dict(lam, resid, history (nblocks, nline, m) device
+    tensors -- history entries of passes skipped by the early exit are NaN --, info)."""
+    L = load_library()
+    p, ld = _block_args(psi, ham.npw, "psi")
+    h, ldh = _block_args(hpsi, ham.npw, "hpsi")
+    nb = int(psi.shape[0])
+    need = int(L.pwh_lobpcg_workspace_bytes(ham.handle, nb, int(nblocks)))
+    if need == 0:
+        raise PwhamError("pwh_lobpcg_workspace_bytes: nband must be a positive multiple of nblocks")
+    lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    res = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    hist = torch.full((int(nblocks), max(int(nline), 0), nb // int(nblocks)), float("nan"), dtype=torch.float64, device=psi.device)
+    info = torch.zeros(1, dtype=torch.int32, device=psi.device)
+    ws = _ws(psi.device, need, tag="lobpcg")
+    with torch.cuda.device(ham.device):
+        _check(L.pwh_lobpcg(ham.handle, nb, int(nblocks), int(nline), float(tol), p, ld, h, ldh, lam.data_ptr(), res.data_ptr(),
+                            hist.data_ptr() if hist.numel() else None, info.data_ptr(), ws.data_ptr(), ws.numel(),
+                            _stream_ptr(ham.device)), "pwh_lobpcg")
+    return {"lam": lam, "resid": res, "history": hist, "info": int(info.item())}
 
 
 # ----------------------------------------------------------------------------------------------------------------

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpwham.so")
-SOURCES = ["pwham.cu", "local_kernels.cu", "local_fast.cu", "local_v2.cu", "local_z.cu", "zgemm.cu", "rr.cu", "rr_api.cu", "paw.cu"]
+SOURCES = ["pwham.cu", "local_kernels.cu", "local_fast.cu", "local_v2.cu", "local_z.cu", "zgemm.cu", "rr.cu", "rr_api.cu", "paw.cu", "lobpcg.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-shared"]
 

@@ -2,6 +2,8 @@
 #pragma once
 #include "common.cuh"
 
+struct pwh_ham;   // the opaque handle of include/pwham.h (defined in pwham.cu)
+
 namespace pwh {
 
 void count_launch();
@@ -105,6 +107,9 @@ void launch_mat_axpby(int n, double alpha, c128* A, int64_t lda, double beta, co
 // out = alpha (z - c y) - beta yprev  (yprev may be null; out may alias z or yprev)
 void launch_cheb_axpy(int64_t npw, int64_t nband, const c128* z, int64_t ldz, const c128* y, int64_t ldy, const c128* yprev,
                       int64_t ldp, c128* out, int64_t ldo, double alpha, double cshift, double beta, cudaStream_t st);
+
+// pwham.cu: the kinetic diagonal kin[npw] of a handle (device pointer)
+const double* ham_kin(const ::pwh_ham* ham);
 
 // pwham.cu: records the thread-local error message of the C ABI and returns `code`
 int api_fail(int code, const char* fmt, ...);

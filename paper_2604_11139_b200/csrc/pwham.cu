@@ -647,6 +647,10 @@ extern "C" int pwh_ham_setup(pwh_ham** out, const double lattice[9], const doubl
   return PWH_OK;
 }
 
+namespace pwh {
+const double* ham_kin(const pwh_ham* h) { return h->lp.kin; }
+}  // namespace pwh
+
 extern "C" int pwh_ham_info(const pwh_ham* h, int64_t info[8]) {
   if (!h || !info) return fail(PWH_EINVAL, "null argument");
   info[0] = h->npw; info[1] = h->nproj; info[2] = h->n1; info[3] = h->n2; info[4] = h->n3;

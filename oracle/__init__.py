@@ -7,6 +7,7 @@ never imports it.  See oracle/pw_oracle.c for the definitions and citations, DES
 from .pw_oracle import (apply_h, build, cheb_filter, dft1d, dft3d, fft1d, gram, kinetic, n_threads,  # noqa: F401
                         TERM_KIN, TERM_LOC, TERM_NL, TERM_ALL)
 from .dense import dense_h  # noqa: F401
+from . import density_oracle as density_oracle  # noqa: F401   (density, band sharding)
 from . import lobpcg_oracle as lobpcg_oracle  # noqa: F401   (LOBPCG block solve)
 from . import paw_oracle as paw  # noqa: F401   (PAW-style generalised problem)
 from . import rr_oracle as rr  # noqa: F401   (Rayleigh-Ritz companion steps)

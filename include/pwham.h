@@ -301,6 +301,28 @@ int pwh_lobpcg(pwh_ham* ham, int64_t nband, int64_t nblocks, int nline, double t
                int64_t ldh, double* lambda, double* resid, double* history, int32_t* info, void* ws, size_t ws_bytes,
                void* stream);
 
+/*
+ * ---------------------------------------------------------------------------------------------------------------
+ * Electronic density (Algorithm 3 steps 9-10: "for every k-point: accumulate electronic density from f, Psi
+ * for current k-point (FFT on GPU)").  It reuses the scatter and the inverse half of the local-potential
+ * transforms.
+ * ---------------------------------------------------------------------------------------------------------------
+ *
+ * pwh_density_accumulate -- rho(r) += weight * sum_i occ[i] |u_i(r)|^2 with u_i(r) = sum_G psi_i(G) exp(+2 pi i n_G.r/n), the
+ * unnormalised inverse transform of the local-potential step (readings R6, R17: the paper prints no formula;
+ * `weight` carries the caller's convention, e.g. w_k / Omega, with which sum_r rho(r) Omega / F = sum_k w_k sum_i occ_i for
+ * orthonormal bands).
+ *   psi   [in]     npw x nband, leading dimension ld;   occ [in] DEVICE nband doubles (occupations f_i);
+ *   rho   [in/out] DEVICE double [n1*n2*n3], index i1 + n1*(i2 + n2*i3) like vloc; ACCUMULATED, so one array collects the
+ *                  bands of several calls and the k-points of several handles (zero it first).
+ *   ws / ws_bytes  at least pwh_density_workspace_bytes(ham, nband), 256-byte aligned.
+ * The sum over the bands of one call is formed in band order by one owner thread per grid point: the result is
+ * deterministic.  Errors: PWH_EINVAL (null pointer, ld < npw, workspace too small or misaligned), PWH_ECUDA.
+ */
+size_t pwh_density_workspace_bytes(const pwh_ham* ham, int64_t nband_max);
+int pwh_density_accumulate(pwh_ham* ham, int64_t nband, const pwh_c128* psi, int64_t ld, const double* occ, double weight,
+                           double* rho, void* ws, size_t ws_bytes, void* stream);
+
 /* Number of kernel launches issued by this library since load (all handles, all threads). */
 int64_t pwh_launch_count(void);
 

@@ -28,7 +28,8 @@ EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply
            "pwh_heev", "pwh_hegv", "pwh_rr_workspace_bytes", "pwh_chol_ortho", "pwh_rayleigh_ritz",
            "pwh_chebfi_workspace_bytes", "pwh_chebfi_iteration",
            "pwh_ham_set_paw", "pwh_apply_hs", "pwh_apply_sinv", "pwh_cheb_filter_gen",
-           "pwh_lobpcg_workspace_bytes", "pwh_lobpcg"]
+           "pwh_lobpcg_workspace_bytes", "pwh_lobpcg",
+           "pwh_density_workspace_bytes", "pwh_density_accumulate"]
 
 STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "colstats", "dense_small",
           "jacobi", "axpy", "reserved10", "reserved11"]
@@ -118,6 +119,10 @@ def load_library() -> ctypes.CDLL:
     L.pwh_apply_sinv.restype = i32
     L.pwh_cheb_filter_gen.argtypes = [vp, i64, vp, i64, i32, dbl, dbl, dbl, vp, sz, vp]
     L.pwh_cheb_filter_gen.restype = i32
+    L.pwh_density_workspace_bytes.argtypes = [vp, i64]
+    L.pwh_density_workspace_bytes.restype = sz
+    L.pwh_density_accumulate.argtypes = [vp, i64, vp, i64, vp, dbl, vp, vp, sz, vp]
+    L.pwh_density_accumulate.restype = i32
     L.pwh_lobpcg_workspace_bytes.argtypes = [vp, i64, i64]
     L.pwh_lobpcg_workspace_bytes.restype = sz
     L.pwh_lobpcg.argtypes = [vp, i64, i64, i32, dbl, vp, i64, vp, i64, vp, vp, vp, vp, vp, sz, vp]
@@ -261,6 +266,27 @@ def cheb_filter(ham: Ham, psi: torch.Tensor, degree: int, a: float, b: float, a0
                                ws.numel(), _stream_ptr(ham.device))
     _check(rc, "pwh_cheb_filter")
     return psi
+
+
+def density_accumulate(ham: Ham, psi: torch.Tensor, occ, rho: torch.Tensor, weight: float = 1.0) -> torch.Tensor:
+    """pwh_density_accumulate: rho (n3, n2, n1) float64 += weight * sum_i occ[i] |u_i(r)|^2 for the block psi; returns rho."""
+    L = load_library()
+    p_ptr, ld = _block_args(psi, ham.npw, "psi")
+    nband = int(psi.shape[0])
+    f = _dev_tensor(occ if isinstance(occ, torch.Tensor) else np.asarray(occ, dtype=np.float64), torch.float64, ham.device)
+    info = ham.info()
+    if f.dim() != 1 or f.shape[0] != nband:
+        raise PwhamError("occ must have shape (nband,)")
+    if not (rho.is_cuda and rho.dtype == torch.float64 and rho.is_contiguous()
+            and tuple(rho.shape) == (info["n3"], info["n2"], info["n1"])):
+        raise PwhamError("rho must be a contiguous CUDA float64 tensor of shape (n3, n2, n1)")
+    need = int(L.pwh_density_workspace_bytes(ham.handle, nband))
+    ws = torch.empty(need, dtype=torch.uint8, device=ham.device)
+    with torch.cuda.device(ham.device):
+        rc = L.pwh_density_accumulate(ham.handle, nband, p_ptr, ld, f.data_ptr(), float(weight), rho.data_ptr(),
+                                      ws.data_ptr(), ws.numel(), _stream_ptr(ham.device))
+    _check(rc, "pwh_density_accumulate")
+    return rho
 
 
 _gram_ws = {}

@@ -31,6 +31,10 @@ void launch_zfwd_gather(const LocalPlan& P, const c128* colbuf, const c128* y, i
                         int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
                         cudaStream_t st);
 
+void launch_density_plane(const LocalPlan& P, const c128* colbuf, int nb, const double* occ, double* acc, cudaStream_t st);
+void launch_density_unpermute(const LocalPlan& P, const double* acc, const int* natx, const int* naty, const int* natz,
+                              double weight, double* rho, cudaStream_t st);
+
 // local_fast.cu
 size_t fast_zkernel_smem(const FastPlan& P);
 size_t fast_plane_smem(const FastPlan& P);
@@ -40,6 +44,9 @@ void launch_fast_plane(const FastPlan& P, c128* colbuf, int nb, cudaStream_t st)
 void launch_fast_zfwd_gather(const FastPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,
                              int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
                              cudaStream_t st);
+
+void launch_fast_density_plane(const FastPlan& P, const c128* colbuf, int nb, const double* occ, double* acc, cudaStream_t st);
+void launch_fast_density_unslot(const FastPlan& P, const double* acc, double weight, double* rho, cudaStream_t st);
 
 // local_v2.cu
 bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max);

@@ -329,6 +329,126 @@ __global__ void __launch_bounds__(PT_MAX, 1) kf_plane(const FastPlan P, c128* __
   for (int c = tid; c < P.ncols; c += nthr) plane[c] = half[P.col_hp[c]];
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// density accumulation (Algorithm 3 step 10)
+// ---------------------------------------------------------------------------------------------------------------
+// One CTA per z-slot walks over the bands of the group in order: disc -> inverse y -> inverse x (the first half of
+// kf_plane), then acc[zslot][xslot][yslot] += occ[band] |u|^2.  A real-space point is owned by one thread of one CTA and
+// the bands come in a fixed order, so the sum is deterministic.  acc is in slot order; kf_density_unslot adds it to the
+// caller's array in natural order.
+__global__ void __launch_bounds__(PT_MAX, 1) kf_density_plane(const FastPlan P, const c128* __restrict__ colbuf, int nb,
+                                                              const double* __restrict__ occ, double* __restrict__ acc) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  c128* half = reinterpret_cast<c128*>(smem_raw);
+  c128* T = half + P.nxl * P.ystride;
+  c128* twx = T + P.tsize;
+  c128* twy = twx + P.n1;
+  short* xl_of_x = reinterpret_cast<short*>(twy + P.n2);
+  const int tid = threadIdx.x, nthr = blockDim.x, zslot = blockIdx.x;
+  const int ys = P.ystride, nxl = P.nxl, YB = P.yb;
+  const int r1x = P.r1[0], r2x = P.r2[0], r1y = P.r1[1], r2y = P.r2[1];
+  const int n2 = P.n2;
+  copy_tw(twx, P.tw[0], P.n1, tid, nthr);
+  copy_tw(twy, P.tw[1], P.n2, tid, nthr);
+  for (int i = tid; i < P.n1; i += nthr) xl_of_x[i] = P.xl_of_x[i];
+  double* __restrict__ az = acc + (int64_t)zslot * P.n1 * P.n2;   // [xslot][yslot]
+  const int nhalf = nxl * ys;
+  for (int band = 0; band < nb; ++band) {
+    const double f = occ[band];
+    __syncthreads();
+    for (int i = tid; i < nhalf; i += nthr) half[i] = cmake(0.0, 0.0);
+    __syncthreads();
+    const c128* plane = colbuf + ((int64_t)band * P.n3 + zslot) * P.ncols_pad;
+    for (int c = tid; c < P.ncols; c += nthr) half[P.col_hp[c]] = plane[c];
+    __syncthreads();
+    with_radix<true>(r1y, [&](auto rc) {
+      constexpr int R = decltype(rc)::value;
+      if (r2y == 1)
+        run_pass<R, +1, false>(1, nxl, P.div_nxl, twy, tid, nthr,
+                               [&](int, int q, int l) { return half[l * ys + q]; },
+                               [&](int, int q, int l, c128 v) { half[l * ys + q] = v; });
+      else
+        run_pass<R, +1, true>(r2y, nxl, P.div_nxl, twy, tid, nthr,
+                              [&](int sub, int q, int l) { return half[l * ys + q * r2y + sub]; },
+                              [&](int sub, int q, int l, c128 v) { half[l * ys + q * r2y + sub] = v; });
+    });
+    __syncthreads();
+    if (r2y > 1) {
+      with_radix<false>(r2y, [&](auto rc) {
+        constexpr int R = decltype(rc)::value;
+        run_pass<R, +1, false>(r1y, nxl, P.div_nxl, twy, tid, nthr,
+                               [&](int sub, int q, int l) { return half[l * ys + sub * r2y + q]; },
+                               [&](int sub, int q, int l, c128 v) { half[l * ys + sub * r2y + q] = v; });
+      });
+      __syncthreads();
+    }
+    for (int y0 = 0; y0 < n2; y0 += YB) {
+      if (r2x == 1) {
+        with_radix<true>(r1x, [&](auto rc) {
+          constexpr int R = decltype(rc)::value;
+          for (int yb = tid; yb < YB; yb += nthr) {
+            c128 v[R];
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+              const int xl = xl_of_x[q];
+              v[q] = xl >= 0 ? half[xl * ys + y0 + yb] : cmake(0.0, 0.0);
+            }
+            Dft<R, +1>::run(v);
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+              double* a = az + (int64_t)q * n2 + y0 + yb;
+              *a = fma(f, fma(v[q].x, v[q].x, v[q].y * v[q].y), *a);
+            }
+          }
+        });
+        continue;
+      }
+      with_radix<true>(r1x, [&](auto rc) {
+        constexpr int R = decltype(rc)::value;
+        run_pass<R, +1, true>(r2x, YB, P.div_yb, twx, tid, nthr,
+                              [&](int sub, int q, int yb) {
+                                const int xl = xl_of_x[q * r2x + sub];
+                                return xl >= 0 ? half[xl * ys + y0 + yb] : cmake(0.0, 0.0);
+                              },
+                              [&](int sub, int q, int yb, c128 v) { T[(q * r2x + sub) * YB + yb] = v; });
+      });
+      __syncthreads();
+      with_radix<false>(r2x, [&](auto rc) {
+        constexpr int R = decltype(rc)::value;
+        const int total = r1x * YB;
+        for (int i = tid; i < total; i += nthr) {
+          uint32_t k1, yb;
+          P.div_yb.divmod((uint32_t)i, k1, yb);
+          const c128* t = T + (k1 * r2x) * YB + yb;
+          c128 v[R];
+#pragma unroll
+          for (int q = 0; q < R; ++q) v[q] = t[q * YB];
+          Dft<R, +1>::run(v);
+          double* a = az + (int64_t)(k1 * r2x) * n2 + y0 + yb;
+#pragma unroll
+          for (int q = 0; q < R; ++q) a[(int64_t)q * n2] = fma(f, fma(v[q].x, v[q].x, v[q].y * v[q].y), a[(int64_t)q * n2]);
+        }
+      });
+      __syncthreads();
+    }
+  }
+}
+
+// rho[x + n1 (y + n2 z)] += weight * acc[(zs n1 + xs) n2 + ys]  with the slot maps of k_slot_vloc (pwham.cu)
+__global__ void kf_density_unslot(int n1, int n2, int n3, int r1x, int r2x, int r1y, int r2y, int r1z, int r2z,
+                                  const double* __restrict__ acc, double weight, double* __restrict__ rho) {
+  const int64_t total = (int64_t)n1 * n2 * n3;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int ys = (int)(i % n2);
+    const int xs = (int)((i / n2) % n1);
+    const int zs = (int)(i / ((int64_t)n1 * n2));
+    const int x = xs / r2x + r1x * (xs % r2x), y = ys / r2y + r1y * (ys % r2y), z = zs / r2z + r1z * (zs % r2z);
+    double* r = rho + x + (int64_t)n1 * (y + (int64_t)n2 * z);
+    *r = fma(weight, acc[i], *r);
+  }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -345,7 +465,9 @@ cudaError_t fast_kernels_init(const FastPlan& P) {
   if (e != cudaSuccess) return e;
   e = set_max_dyn_smem(reinterpret_cast<const void*>(&kf_zfwd_gather));
   if (e != cudaSuccess) return e;
-  return set_max_dyn_smem(reinterpret_cast<const void*>(&kf_plane));
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&kf_plane));
+  if (e != cudaSuccess) return e;
+  return set_max_dyn_smem(reinterpret_cast<const void*>(&kf_density_plane));
 }
 
 void launch_fast_scatter_zinv(const FastPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st) {
@@ -358,6 +480,17 @@ void launch_fast_plane(const FastPlan& P, c128* colbuf, int nb, cudaStream_t st)
   dim3 grid(P.n3, nb);
   ScopedLaunch sl(ST_PLANE, st);
   kf_plane<<<grid, P.plane_threads, fast_plane_smem(P), st>>>(P, colbuf);
+}
+
+void launch_fast_density_plane(const FastPlan& P, const c128* colbuf, int nb, const double* occ, double* acc, cudaStream_t st) {
+  ScopedLaunch sl(ST_PLANE, st);
+  kf_density_plane<<<P.n3, P.plane_threads, fast_plane_smem(P), st>>>(P, colbuf, nb, occ, acc);
+}
+
+void launch_fast_density_unslot(const FastPlan& P, const double* acc, double weight, double* rho, cudaStream_t st) {
+  ScopedLaunch sl(ST_AXPY, st);
+  kf_density_unslot<<<148 * 4, 256, 0, st>>>(P.n1, P.n2, P.n3, P.r1[0], P.r2[0], P.r1[1], P.r2[1], P.r1[2], P.r2[2], acc, weight,
+                                             rho);
 }
 
 void launch_fast_zfwd_gather(const FastPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,

@@ -144,6 +144,70 @@ __global__ void __launch_bounds__(PT) k_plane(const LocalPlan P, c128* __restric
   for (int c = tid; c < P.ncols; c += PT) plane[c] = half[P.col_hp[c]];
 }
 
+// Density accumulation on the generic stage plan (Algorithm 3 step 10): one CTA per
+// z position walks over the bands of the group in order: disc -> inverse y -> inverse x, acc[pz][py][px] += occ |u|^2 in
+// digit-permuted positions (deterministic: one owner thread per point, bands in order); k_density_unpermute adds acc to
+// the caller's array in natural order.
+__global__ void __launch_bounds__(PT) k_density_plane(const LocalPlan P, const c128* __restrict__ colbuf, int nb,
+                                                      const double* __restrict__ occ, double* __restrict__ acc) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  c128* half = reinterpret_cast<c128*>(smem_raw);
+  c128* work = half + P.nxl * P.ystride;
+  c128* twx = work + P.xbatch * P.xstride;
+  c128* twy = twx + P.ax[0].tw_len;
+  __shared__ AxisPlan s_ax, s_ay;
+  const int tid = threadIdx.x, pz = blockIdx.x;
+  load_plan(&s_ax, P.axp + 0, tid, PT);
+  load_plan(&s_ay, P.axp + 1, tid, PT);
+  load_tw(twx, P.tw[0], P.ax[0].tw_len, tid, PT);
+  load_tw(twy, P.tw[1], P.ax[1].tw_len, tid, PT);
+  const int nhalf = P.nxl * P.ystride;
+  double* aplane = acc + (int64_t)pz * P.n2 * P.n1;
+  const int xb = P.xbatch;
+  for (int band = 0; band < nb; ++band) {
+    const double f = occ[band];
+    __syncthreads();
+    for (int i = tid; i < nhalf; i += PT) half[i] = cmake(0.0, 0.0);
+    __syncthreads();
+    const c128* plane = colbuf + ((int64_t)band * P.n3 + pz) * P.ncols_pad;
+    for (int c = tid; c < P.ncols; c += PT) half[P.col_hp[c]] = plane[c];
+    __syncthreads();
+    fft_lines<+1>(half, P.nxl, P.div_nxl, P.ystride, s_ay, twy, tid, PT);
+    for (int y0 = 0; y0 < P.n2; y0 += xb) {
+      for (int i = tid; i < xb * P.n1; i += PT) {
+        uint32_t x, yb;
+        P.div_xbatch.divmod((uint32_t)i, x, yb);
+        const int xl = P.xl_of_x[x];
+        work[yb * P.xstride + x] = xl >= 0 ? half[xl * P.ystride + y0 + yb] : cmake(0.0, 0.0);
+      }
+      __syncthreads();
+      fft_lines<+1>(work, xb, P.div_xbatch, P.xstride, s_ax, twx, tid, PT);
+      for (int i = tid; i < xb * P.n1; i += PT) {
+        uint32_t yb, px;
+        P.div_n1.divmod((uint32_t)i, yb, px);
+        const c128 u = work[yb * P.xstride + px];
+        double* a = aplane + (y0 + yb) * P.n1 + px;
+        *a = fma(f, fma(u.x, u.x, u.y * u.y), *a);
+      }
+      __syncthreads();
+    }
+  }
+}
+
+// rho[natx[px] + n1 (naty[py] + n2 natz[pz])] += weight * acc[px + n1 (py + n2 pz)]   (inverse of k_permute_vloc, pwham.cu)
+__global__ void k_density_unpermute(int n1, int n2, int n3, const double* __restrict__ acc, const int* __restrict__ natx,
+                                    const int* __restrict__ naty, const int* __restrict__ natz, double weight,
+                                    double* __restrict__ rho) {
+  const int64_t total = (int64_t)n1 * n2 * n3;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int px = (int)(i % n1);
+    const int py = (int)((i / n1) % n2);
+    const int pz = (int)(i / ((int64_t)n1 * n2));
+    double* r = rho + natx[px] + (int64_t)n1 * (naty[py] + (int64_t)n2 * natz[pz]);
+    *r = fma(weight, acc[i], *r);
+  }
+}
+
 size_t zkernel_smem(const LocalPlan& P) {
   return sizeof(c128) * ((size_t)P.colgrp * P.zstride + P.ax[2].tw_len);
 }
@@ -157,7 +221,9 @@ cudaError_t local_kernels_init(const LocalPlan& P) {
   if (e != cudaSuccess) return e;
   e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zfwd_gather));
   if (e != cudaSuccess) return e;
-  return set_max_dyn_smem(reinterpret_cast<const void*>(&k_plane));
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_plane));
+  if (e != cudaSuccess) return e;
+  return set_max_dyn_smem(reinterpret_cast<const void*>(&k_density_plane));
 }
 
 void launch_scatter_zinv(const LocalPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st) {
@@ -170,6 +236,17 @@ void launch_plane(const LocalPlan& P, c128* colbuf, int nb, cudaStream_t st) {
   dim3 grid(P.n3, nb);
   ScopedLaunch sl(ST_PLANE, st);
   k_plane<<<grid, PT, plane_smem(P), st>>>(P, colbuf);
+}
+
+void launch_density_plane(const LocalPlan& P, const c128* colbuf, int nb, const double* occ, double* acc, cudaStream_t st) {
+  ScopedLaunch sl(ST_PLANE, st);
+  k_density_plane<<<P.n3, PT, plane_smem(P), st>>>(P, colbuf, nb, occ, acc);
+}
+
+void launch_density_unpermute(const LocalPlan& P, const double* acc, const int* natx, const int* naty, const int* natz,
+                              double weight, double* rho, cudaStream_t st) {
+  ScopedLaunch sl(ST_AXPY, st);
+  k_density_unpermute<<<148 * 4, 256, 0, st>>>(P.n1, P.n2, P.n3, acc, natx, naty, natz, weight, rho);
 }
 
 void launch_zfwd_gather(const LocalPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,

@@ -121,6 +121,7 @@ struct pwh_ham {
   ProjMaps pmaps;
   double* dij = nullptr;
   int band_group = 1;
+  const int* dnat[3] = {nullptr, nullptr, nullptr};   // generic stage plan: position -> natural index per axis
   // PAW-style generalised problem (pwh_ham_set_paw): per-atom dense D^R / Q^R blocks and K of S^-1 = I - P K P^H
   bool paw = false;
   int* blk_of = nullptr;         // [nproj] block (atom) of each projector
@@ -139,6 +140,11 @@ struct pwh_ham {
   // copy streams and events of the pipelined host entry points
   cudaStream_t cs_in = nullptr, cs_out = nullptr;
   std::vector<cudaEvent_t> evs;
+  // the band groups of the local stage alternate between two internal streams (each with its own column buffer), so that
+  // the partial last wave of one group's kernels is filled by the other group's (lways = 1: one stream, in order)
+  int lways = 1;
+  cudaStream_t ls[2] = {nullptr, nullptr};
+  cudaEvent_t lev_fork = nullptr, lev_join[2] = {nullptr, nullptr};
 };
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -282,6 +288,11 @@ extern "C" int pwh_ham_destroy(pwh_ham* h) {
   if (h->cs_in) cudaStreamDestroy(h->cs_in);
   if (h->cs_out) cudaStreamDestroy(h->cs_out);
   for (cudaEvent_t e : h->evs) cudaEventDestroy(e);
+  for (int i = 0; i < 2; ++i) {
+    if (h->ls[i]) cudaStreamDestroy(h->ls[i]);
+    if (h->lev_join[i]) cudaEventDestroy(h->lev_join[i]);
+  }
+  if (h->lev_fork) cudaEventDestroy(h->lev_fork);
   delete h;
   return PWH_OK;
 }
@@ -575,7 +586,7 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     CUDA_TRY(fast_kernels_init(fp));
   } else {
     // generic path: V_loc / F in digit-permuted positions
-    const int* dnat[3];
+    const int** dnat = h->dnat;
     for (int ax = 0; ax < 3; ++ax)
       if ((rc = upload(h, nat[ax], &dnat[ax], st))) return rc;
     double* vp = nullptr;
@@ -620,6 +631,14 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     if (eff >= best_eff + 0.005 || (eff >= best_eff - 0.005 && c > grp && eff >= 0.97)) { best_eff = std::max(eff, best_eff); grp = c; }
   }
   h->band_group = (int)grp;
+  h->lways = env_on("PWH_LOCAL_ONE_STREAM") ? 1 : 2;
+  if (h->lways == 2) {
+    for (int i = 0; i < 2; ++i) {
+      CUDA_TRY(cudaStreamCreateWithFlags(&h->ls[i], cudaStreamNonBlocking));
+      CUDA_TRY(cudaEventCreateWithFlags(&h->lev_join[i], cudaEventDisableTiming));
+    }
+    CUDA_TRY(cudaEventCreateWithFlags(&h->lev_fork, cudaEventDisableTiming));
+  }
 
   CUDA_TRY(cudaStreamSynchronize(st));
   return PWH_OK;
@@ -678,7 +697,7 @@ extern "C" int pwh_ham_kernels(const pwh_ham* h, char* buf, size_t n) {
 // workspace
 // ---------------------------------------------------------------------------------------------------------------
 struct WsLayout {
-  size_t colbuf, cmat, part, y1, y2, total;
+  size_t colbuf, colbuf_bytes, cmat, part, y1, y2, total;
   int64_t ldw;
   int group;
 };
@@ -691,7 +710,8 @@ static WsLayout ws_layout(const pwh_ham* h, int64_t nband) {
   w.group = (int)std::min<int64_t>(h->band_group, std::max<int64_t>(nband, 1));
   w.ldw = (int64_t)align_up((size_t)h->npw, 16);
   size_t off = 0;
-  w.colbuf = off; off += align_up((size_t)w.group * h->n3 * h->lp.ncols_pad * sizeof(c128), 256);
+  w.colbuf_bytes = align_up((size_t)w.group * h->n3 * h->lp.ncols_pad * sizeof(c128), 256);
+  w.colbuf = off; off += (size_t)h->lways * w.colbuf_bytes;
   // projections C = P^H Y; with PAW blocks also blockdiag(D) C and blockdiag(Q) C (or K C)
   w.cmat = off;   off += (h->paw ? 3 : 1) * align_up((size_t)std::max<int64_t>(h->nproj, 1) * nband * sizeof(c128), 256);
   w.part = off;   off += align_up(h->nproj > 0 ? zgemm_cn_workspace_upto(h->nproj, nband, h->npw) : 16, 256);
@@ -727,26 +747,41 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
   }
   {
     NvtxRange r("pwh:local+kinetic+recurrence");
-    for (int64_t b0 = 0; b0 < nband; b0 += w.group) {
+    // two-way interleave of the band groups (bands never interact); one stream while the per-launch
+    // profile is on, so that the per-kernel event times are those of kernels running alone
+    const int ways = (h->lways == 2 && nband > w.group && !g_prof_on.load(std::memory_order_relaxed)) ? 2 : 1;
+    if (ways == 2) {
+      CUDA_TRY(cudaEventRecord(h->lev_fork, st));
+      for (int i = 0; i < 2; ++i) CUDA_TRY(cudaStreamWaitEvent(h->ls[i], h->lev_fork, 0));
+    }
+    int64_t gi = 0;
+    for (int64_t b0 = 0; b0 < nband; b0 += w.group, ++gi) {
       const int nb = (int)std::min<int64_t>(w.group, nband - b0);
+      cudaStream_t ls = ways == 2 ? h->ls[gi & 1] : st;
+      c128* cb = ways == 2 ? reinterpret_cast<c128*>(ws + w.colbuf + (size_t)(gi & 1) * w.colbuf_bytes) : colbuf;
       if (h->fast) {
-        if (h->zw) launch_zw_scatter_zinv(h->zp, y + b0 * ldy, ldy, colbuf, nb, st);
-        else launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, colbuf, nb, st);
-        if (h->v2) launch_v2_plane(h->vp, colbuf, nb, st);
-        else launch_fast_plane(h->fp, colbuf, nb, st);
+        if (h->zw) launch_zw_scatter_zinv(h->zp, y + b0 * ldy, ldy, cb, nb, ls);
+        else launch_fast_scatter_zinv(h->fp, y + b0 * ldy, ldy, cb, nb, ls);
+        if (h->v2) launch_v2_plane(h->vp, cb, nb, ls);
+        else launch_fast_plane(h->fp, cb, nb, ls);
         if (h->zw)
-          launch_zw_zfwd_gather(h->zp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
-                                out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+          launch_zw_zfwd_gather(h->zp, cb, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                                out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, ls);
         else
-          launch_fast_zfwd_gather(h->fp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
-                                  out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+          launch_fast_zfwd_gather(h->fp, cb, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                                  out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, ls);
       } else {
-        launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, colbuf, nb, st);
-        launch_plane(h->lp, colbuf, nb, st);
-        launch_zfwd_gather(h->lp, colbuf, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
-                           out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, st);
+        launch_scatter_zinv(h->lp, y + b0 * ldy, ldy, cb, nb, ls);
+        launch_plane(h->lp, cb, nb, ls);
+        launch_zfwd_gather(h->lp, cb, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
+                           out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, ls);
       }
     }
+    if (ways == 2)
+      for (int i = 0; i < 2; ++i) {
+        CUDA_TRY(cudaEventRecord(h->lev_join[i], h->ls[i]));
+        CUDA_TRY(cudaStreamWaitEvent(st, h->lev_join[i], 0));
+      }
   }
   if (h->nproj > 0) {
     NvtxRange r("pwh:nonlocal:Y+=a.P.C");
@@ -829,6 +864,59 @@ extern "C" int pwh_cheb_filter(pwh_ham* h, int64_t nband, pwh_c128* psi, int64_t
     if (rc) return rc;
     sigma = sigma_new;
   }
+  return PWH_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// electronic density (Algorithm 3 step 10)
+// ---------------------------------------------------------------------------------------------------------------
+struct DensLayout { size_t colbuf, acc, total; int group; };
+static DensLayout dens_layout(const pwh_ham* h, int64_t nband) {
+  DensLayout d;
+  d.group = (int)std::min<int64_t>(h->band_group, std::max<int64_t>(nband, 1));
+  size_t off = 0;
+  d.colbuf = off; off += align_up((size_t)d.group * h->n3 * h->lp.ncols_pad * sizeof(c128), 256);
+  d.acc = off;    off += align_up((size_t)h->n1 * h->n2 * h->n3 * sizeof(double), 256);
+  d.total = off;
+  return d;
+}
+
+extern "C" size_t pwh_density_workspace_bytes(const pwh_ham* h, int64_t nband_max) {
+  if (!h || nband_max < 0) return 0;
+  return dens_layout(h, std::max<int64_t>(nband_max, 1)).total;
+}
+
+extern "C" int pwh_density_accumulate(pwh_ham* h, int64_t nband, const pwh_c128* psi, int64_t ld, const double* occ,
+                                      double weight, double* rho, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return fail(PWH_EINVAL, "handle is null");
+  if (nband < 0) return fail(PWH_EINVAL, "nband < 0");
+  if (nband == 0) return PWH_OK;
+  if (!psi || !occ || !rho) return fail(PWH_EINVAL, "psi / occ / rho null");
+  if (ld < h->npw) return fail(PWH_EINVAL, "ld < npw");
+  if (!ws || (uintptr_t)ws % 256 != 0) return fail(PWH_EINVAL, "workspace null or not 256-byte aligned");
+  const DensLayout d = dens_layout(h, nband);
+  if (ws_bytes < d.total) return fail(PWH_EINVAL, "workspace too small: %zu < %zu bytes", ws_bytes, d.total);
+  NvtxRange r("pwh_density_accumulate");
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned char* wsb = reinterpret_cast<unsigned char*>(ws);
+  c128* colbuf = reinterpret_cast<c128*>(wsb + d.colbuf);
+  double* acc = reinterpret_cast<double*>(wsb + d.acc);
+  const c128* y = reinterpret_cast<const c128*>(psi);
+  CUDA_TRY(cudaMemsetAsync(acc, 0, (size_t)h->n1 * h->n2 * h->n3 * sizeof(double), st));
+  for (int64_t b0 = 0; b0 < nband; b0 += d.group) {
+    const int nb = (int)std::min<int64_t>(d.group, nband - b0);
+    if (h->fast) {
+      if (h->zw) launch_zw_scatter_zinv(h->zp, y + b0 * ld, ld, colbuf, nb, st);
+      else launch_fast_scatter_zinv(h->fp, y + b0 * ld, ld, colbuf, nb, st);
+      launch_fast_density_plane(h->fp, colbuf, nb, occ + b0, acc, st);
+    } else {
+      launch_scatter_zinv(h->lp, y + b0 * ld, ld, colbuf, nb, st);
+      launch_density_plane(h->lp, colbuf, nb, occ + b0, acc, st);
+    }
+  }
+  if (h->fast) launch_fast_density_unslot(h->fp, acc, weight, rho, st);
+  else launch_density_unpermute(h->lp, acc, h->dnat[0], h->dnat[1], h->dnat[2], weight, rho, st);
+  CUDA_TRY(cudaGetLastError());
   return PWH_OK;
 }
 

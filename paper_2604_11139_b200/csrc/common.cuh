@@ -108,7 +108,8 @@ struct V2Plan {
   int zcol;                  // first padding column (>= ncols): zero on input; zcol + 1 takes the stores outside the disc
   int variant;               // which template instantiation
   int r1[2], r2[2], nyb;     // x, y radices and y-slots per warp batch of that instantiation
-  const int2* yrow;          // [n2] per wrapped y: .x = first column - xlmin, .y = xlmin | (count << 16)
+  const int2* yrow;          // [n2] per y-row yl = (y - y0) mod n2, y0 the lowest touched row: .x = first column - xlmin,
+                             // .y = xlmin | (count << 16)
   const c128* twA[2];        // x, y: [r2][r1+1]  exp(+2 pi i s k1 / n) at s (r1+1) + k1
   const c128* twB[2];        // x, y: [r1][r2+1]  the same value at k1 (r2+1) + s
   const double* vperm;       // V_loc/F in kernel read order (kv2_perm_vloc)
@@ -118,13 +119,15 @@ struct V2Plan {
 // Plan of the warp-private z kernels (local_z.cu): n3 = r1 * r2, a work item is (cw columns, one band).
 struct ZPlan {
   int n3, r1, r2;
-  int r1p;                   // r1 rounded up to a multiple of 4 (row length of ztab)
+  int lq;                    // z-rows zl = q r2 + sub with q >= lq are outside the sphere (lq = r1: no pruning)
+  int lqp;                   // lq rounded up to a multiple of 4 (row length of ztab)
   int cw, log2cw;            // columns per work item (power of two: 4 when r2 >= 6), its log2
   int nq;                    // work items per band = ncols_pad / cw
   int ncols_pad;
   int zs;                    // elements per column of a warp buffer; position of z = q r2 + s is q (r2 + 1) + s
-  const int* ztab;           // [nq][r1p/4][r2*cw][4]: plane-wave index of column quad*cw + c at z = q r2 + sub (element
-                             // sub*cw + c, q = 4 j + k), -1 outside the sphere
+  const int* ztab;           // [nq][lqp/4][r2*cw][4]: plane-wave index of column quad*cw + c at z-row zl = q r2 + sub, counted
+                             // from the lowest touched z: zl = (z - z0) mod n3 (element sub*cw + c, q = 4 j + k), -1 outside
+                             // the sphere
   const c128* tw;            // tw[t] = exp(+2 pi i t / n3)
   const double* kin;         // [npw]
 };

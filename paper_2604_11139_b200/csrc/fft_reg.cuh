@@ -184,4 +184,99 @@ template <int DIR> struct Dft<12, DIR> { __device__ __forceinline__ static void 
 template <int DIR> struct Dft<15, DIR> { __device__ __forceinline__ static void run(c128* v) { DftCT<3, 5, DIR>::run(v); } };
 template <int DIR> struct Dft<16, DIR> { __device__ __forceinline__ static void run(c128* v) { DftCT<4, 4, DIR>::run(v); } };
 
+// ---- pruned transforms -------------------------------------------------------------------------------------------------
+// The sphere occupies a prefix of every spectral axis once the axis is indexed from its lowest touched line (a shift of the
+// spectral index is a phase in real space, which cancels between the inverse and the forward transform around the real,
+// pointwise V_loc multiply).  In the strided-role pass of n = R * r2 the inputs of one radix-R transform are the lines
+// s + r2 q: only q < L = ceil(touched / r2) can be non-zero on the way in, and only those outputs are wanted on the way out.
+
+// v0 + exp(DIR 2 pi i K / N) v1 with compile-time K, N
+template <int K, int N, int DIR>
+__device__ __forceinline__ c128 add_rot(c128 v0, c128 v1) {
+  constexpr int k = ((K % N) + N) % N;
+  if constexpr (k == 0 || 4 * k == N || 2 * k == N || 4 * k == 3 * N) return cadd(v0, rot<K, N, DIR>(v1));
+  else {
+    constexpr double c = cos_turn(k, N);
+    constexpr double s = (DIR > 0 ? 1.0 : -1.0) * sin_turn(k, N);
+    return cmake(fma(c, v1.x, fma(-s, v1.y, v0.x)), fma(c, v1.y, fma(s, v1.x, v0.y)));
+  }
+}
+
+// DFT of length A whose inputs v[LA..A-1] are zero (they are neither read nor assumed initialised); all A outputs
+template <int A, int DIR, int LA>
+struct DftIn {
+  template <int K>
+  __device__ __forceinline__ static void two(c128 v0, c128 v1, c128* v) {
+    if constexpr (K < A) {
+      v[K] = add_rot<K, A, DIR>(v0, v1);
+      two<K + 1>(v0, v1, v);
+    }
+  }
+  __device__ __forceinline__ static void run(c128* v) {
+    if constexpr (LA <= 0) {
+#pragma unroll
+      for (int k = 0; k < A; ++k) v[k] = cmake(0.0, 0.0);
+    } else if constexpr (LA == 1) {
+#pragma unroll
+      for (int k = 1; k < A; ++k) v[k] = v[0];
+    } else if constexpr (LA == 2 && A > 2) {
+      const c128 v0 = v[0], v1 = v[1];
+      two<0>(v0, v1, v);
+    } else {
+#pragma unroll
+      for (int a = (LA < A ? LA : A); a < A; ++a) v[a] = cmake(0.0, 0.0);
+      Dft<A, DIR>::run(v);
+    }
+  }
+};
+
+// Cooley-Tukey product R = A * B (n = a*B + b, k = ka + A*kb) with inputs n >= L zero: the first-stage transforms over a
+// see only the a with a*B + b < L
+template <int A, int B, int DIR, int L>
+struct DftCTIn {
+  template <int Bi>
+  __device__ __forceinline__ static void first(const c128* v, c128 (*t)[A]) {
+    if constexpr (Bi < B) {
+      constexpr int LA = (L - Bi + B - 1) / B < 0 ? 0 : ((L - Bi + B - 1) / B > A ? A : (L - Bi + B - 1) / B);
+      c128 u[A];
+#pragma unroll
+      for (int a = 0; a < LA; ++a) u[a] = v[a * B + Bi];
+      DftIn<A, DIR, LA>::run(u);
+      if constexpr (LA > 0) DftCT<A, B, DIR>::template twiddle_row<Bi, 0>(u);
+#pragma unroll
+      for (int a = 0; a < A; ++a) t[Bi][a] = u[a];
+      first<Bi + 1>(v, t);
+    }
+  }
+  __device__ __forceinline__ static void run(c128* v) {
+    c128 t[B][A];
+    first<0>(v, t);
+#pragma unroll
+    for (int ka = 0; ka < A; ++ka) {
+      c128 u[B];
+#pragma unroll
+      for (int b = 0; b < B; ++b) u[b] = t[b][ka];
+      Dft<B, DIR>::run(u);
+#pragma unroll
+      for (int kb = 0; kb < B; ++kb) v[ka + A * kb] = u[kb];
+    }
+  }
+};
+
+// v[0..R-1] <- DFT_R(v) where v[L..R-1] are zero on entry (not read)
+template <int R, int DIR, int L>
+struct DftPrunedIn {
+  __device__ __forceinline__ static void run(c128* v) {
+    if constexpr (L >= R) Dft<R, DIR>::run(v);
+    else if constexpr (R == 6) DftCTIn<2, 3, DIR, L>::run(v);
+    else if constexpr (R == 8) DftCTIn<2, 4, DIR, L>::run(v);
+    else if constexpr (R == 9) DftCTIn<3, 3, DIR, L>::run(v);
+    else if constexpr (R == 10) DftCTIn<2, 5, DIR, L>::run(v);
+    else if constexpr (R == 12) DftCTIn<3, 4, DIR, L>::run(v);
+    else if constexpr (R == 15) DftCTIn<3, 5, DIR, L>::run(v);
+    else if constexpr (R == 16) DftCTIn<4, 4, DIR, L>::run(v);
+    else DftIn<R, DIR, L>::run(v);
+  }
+};
+
 }  // namespace pwh

@@ -49,13 +49,14 @@ void launch_fast_density_plane(const FastPlan& P, const c128* colbuf, int nb, co
 void launch_fast_density_unslot(const FastPlan& P, const double* acc, double weight, double* rho, cudaStream_t st);
 
 // local_v2.cu
-bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max);
+bool v2_select(V2Plan& P, int n1, int n2, int nxl, int nyl, size_t smem_max, bool no_prune = false);
 cudaError_t v2_kernels_init(const V2Plan& P);
 void launch_v2_perm_vloc(const V2Plan& P, int r1z, int r2z, const double* vloc, double* out, cudaStream_t st);
 void launch_v2_plane(const V2Plan& P, c128* colbuf, int nb, cudaStream_t st);
 
 // local_z.cu
 size_t zw_smem(const ZPlan& P);
+int zw_pruned_len(int r1);   // rows of the pruned instantiation of a radix-r1 strided-role pass
 cudaError_t zw_kernels_init(const ZPlan& P);
 void launch_zw_scatter_zinv(const ZPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st);
 void launch_zw_zfwd_gather(const ZPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,

@@ -29,13 +29,15 @@ namespace pwh {
 
 namespace {
 
-template <int N1_, int R1X_, int R2X_, int N2_, int R1Y_, int R2Y_, int NW_, int NYB_, int MINB_ = 1>
+template <int N1_, int R1X_, int R2X_, int N2_, int R1Y_, int R2Y_, int NW_, int NYB_, int MINB_ = 1, int LQX_ = R1X_>
 struct PC {
   static constexpr int N1 = N1_, R1X = R1X_, R2X = R2X_, N2 = N2_, R1Y = R1Y_, R2Y = R2Y_, NW = NW_, NYB = NYB_;
   static_assert(R1X * R2X == N1 && R1Y * R2Y == N2, "axis factorisation");
   static_assert(N2 % NYB == 0, "y batches");
   static constexpr int NT = NW * 32;
   static constexpr int MINB = MINB_;                 // CTAs per SM the register budget is capped for
+  static constexpr int LQX = LQX_;                   // x-lines l = s + R2X q with q >= LQX are untouched: nxl <= LQX * R2X
+  static constexpr int LQY = LQX_ * R1Y_ >= R1X_ * R1Y_ ? R1Y_ : (LQX_ < R1Y_ ? LQX_ : R1Y_);   // the same for the y-rows: nyl <= LQY * R2Y
   static constexpr int YS = N2 | 1;                  // odd line stride of the half-plane (elements)
   static constexpr int XP = R1X * (R2X + 1);         // padded length of one x-line in a warp buffer
   static constexpr int TWA_X = R2X * (R1X + 1), TWB_X = R1X * (R2X + 1);
@@ -51,7 +53,7 @@ __device__ __forceinline__ c128 czero() { return cmake(0.0, 0.0); }
 template <class C>
 __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128* __restrict__ colbuf) {
   constexpr int N1 = C::N1, R1X = C::R1X, R2X = C::R2X, N2 = C::N2, R1Y = C::R1Y, R2Y = C::R2Y;
-  constexpr int NT = C::NT, YS = C::YS, XP = C::XP, NYB = C::NYB;
+  constexpr int NT = C::NT, YS = C::YS, XP = C::XP, NYB = C::NYB, LQX = C::LQX, LQY = C::LQY;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nxl = P.nxl;
   c128* half = reinterpret_cast<c128*>(smem_raw);            // [nxl + 2][YS]: line nxl stays zero (read for the
@@ -76,7 +78,8 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
   c128* __restrict__ plane = colbuf + ((int64_t)band * P.n3 + zslot) * P.ncols_pad;
   const int zcol = P.zcol;
 
-  // ---- y1: inverse y, strided role (radix R1Y over y = q R2Y + s), input straight from the disc in global memory
+  // ---- y1: inverse y, strided role (radix R1Y over the y-ROWS yl = q R2Y + s, counted from the lowest touched row: the
+  //      same index shift as in the x direction, so only q < LQY can hold a row of the disc), input straight from the disc
   {
     const int nitems = R2Y * nxl;
     for (int i = tid; i < nitems; i += NT) {
@@ -85,12 +88,12 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
       c128 v[R1Y];
       const int2* yr = yrow + s;
 #pragma unroll
-      for (int q = 0; q < R1Y; ++q) {
+      for (int q = 0; q < LQY; ++q) {
         const int2 row = yr[q * R2Y];
         const uint32_t d = l - (uint32_t)(row.y & 0xffff);
         v[q] = plane[d < (uint32_t)(row.y >> 16) ? row.x + (int)l : zcol];   // zcol: a padding column, always zero
       }
-      Dft<R1Y, +1>::run(v);
+      DftPrunedIn<R1Y, +1, LQY>::run(v);
       const c128* tw = twAy + s * (R1Y + 1);
       c128* dst = half + l * YS + s;
       dst[0] = v[0];
@@ -119,7 +122,6 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
   // ---- x direction, warp-private: NYB y-slots at a time
   {
     c128* tw_ = tbuf + warp * (NYB * XP);
-    const int x0 = P.x0;
     const double* __restrict__ vz = P.vperm + (int64_t)zslot * ((int64_t)N1 * N2);
     constexpr int XG = 32 / R1X;               // y-slots pass (b) handles per round: lane = xg * R1X + xk1
     static_assert(NYB % XG == 0, "pass (b) rounds");
@@ -129,20 +131,32 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
     for (int q = 0; q < R2X; ++q) xtw[q] = twBx[xk1 * (R2X + 1) + q];
     for (int b = warp; b < C::NBATCH; b += C::NW) {
       const int y0 = b * NYB;
-      // (a) strided role: radix R1X over x = q R2X + s, twiddle, into the warp buffer at k1 (R2X+1) + s
+      // V_loc/F of this batch: requested from L2 now, consumed in pass (b) after the radix-R1X transforms of pass (a)
+      const double* __restrict__ vb = vz + (int64_t)b * (R2X * R1X * NYB);
+      double vreg[NYB / XG][R2X];
+#ifndef PWH_V2_NO_PREFETCH
+      if (lane < XG * R1X) {
+#pragma unroll
+        for (int r = 0; r < NYB / XG; ++r)
+#pragma unroll
+          for (int q = 0; q < R2X; ++q) vreg[r][q] = __ldg(vb + q * (R1X * NYB) + xk1 + R1X * (xg + r * XG));
+      }
+#endif
+      // (a) strided role: radix R1X over the x-LINES l = q R2X + s, twiddle, into the warp buffer at k1 (R2X+1) + s.
+      //     The transform runs over the line index l = (x - x0) mod N1 instead of x: the shift is the phase w^(-x0 r) in real
+      //     space, which the forward transform of pass (c) takes out again around the real, pointwise V_loc multiply -- so
+      //     the touched lines are the prefix l < nxl, only the first LQX inputs of a radix-R1X transform can be non-zero
+      //     and nothing wraps.
       for (int i = lane; i < R2X * NYB; i += 32) {
         const int s = i % R2X, yb = i / R2X;
-        int xl = s - x0;                       // x-line of x = s (q = 0), modulo N1
-        if (xl < 0) xl += N1;
         const c128* src = half + y0 + yb;
         c128 v[R1X];
 #pragma unroll
-        for (int q = 0; q < R1X; ++q) {
-          int xq = xl + q * R2X;
-          if (xq >= N1) xq -= N1;
-          v[q] = src[(xq < nxl ? xq : nxl) * YS];
+        for (int q = 0; q < LQX; ++q) {
+          const int l = s + q * R2X;
+          v[q] = src[(l < nxl ? l : nxl) * YS];
         }
-        Dft<R1X, +1>::run(v);
+        DftPrunedIn<R1X, +1, LQX>::run(v);
         c128* dst = tw_ + yb * XP + s;
 #pragma unroll
         for (int q = 0; q < R1X; ++q) dst[q * (R2X + 1)] = v[q];
@@ -151,11 +165,10 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
       // (b) contiguous role: twiddle w^(s k1), radix R2X inverse -> real space, multiply by V_loc/F, radix R2X forward,
       //     twiddle w^-(s k1).  A lane keeps the same k1 for all its items, so its R2X-1 twiddles live in registers and
       //     passes (a) and (c) are plain radix-R1X transforms.
-      const double* __restrict__ vb = vz + (int64_t)b * (R2X * R1X * NYB);
       if (lane < XG * R1X) {
 #pragma unroll
-        for (int yb = xg; yb < NYB; yb += XG) {
-          const int i = xk1 + R1X * yb;
+        for (int r = 0; r < NYB / XG; ++r) {
+          const int yb = xg + r * XG;
           c128* t = tw_ + yb * XP + xk1 * (R2X + 1);
           c128 v[R2X];
           v[0] = t[0];
@@ -163,7 +176,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
           for (int q = 1; q < R2X; ++q) v[q] = cmul(t[q], xtw[q]);
           Dft<R2X, +1>::run(v);
 #pragma unroll
-          for (int q = 0; q < R2X; ++q) v[q] = cscale(vb[q * (R1X * NYB) + i], v[q]);
+#ifdef PWH_V2_NO_PREFETCH
+          for (int q = 0; q < R2X; ++q) vreg[r][q] = vb[q * (R1X * NYB) + xk1 + R1X * yb];
+#pragma unroll
+#endif
+          for (int q = 0; q < R2X; ++q) v[q] = cscale(vreg[r][q], v[q]);
           Dft<R2X, -1>::run(v);
           t[0] = v[0];
 #pragma unroll
@@ -171,11 +188,10 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
         }
       }
       __syncwarp();
-      // (c) strided role: radix R1X forward over k1, keep the touched x-lines
+      // (c) strided role: radix R1X forward over k1; only the outputs q < LQX can be touched lines (the others are never
+      //     stored, so the compiler drops the butterflies that feed only them)
       for (int i = lane; i < R2X * NYB; i += 32) {
         const int s = i % R2X, yb = i / R2X;
-        int xl = s - x0;
-        if (xl < 0) xl += N1;
         const c128* src = tw_ + yb * XP + s;
         c128 v[R1X];
 #pragma unroll
@@ -183,10 +199,9 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
         Dft<R1X, -1>::run(v);
         c128* dst = half + y0 + yb;
 #pragma unroll
-        for (int q = 0; q < R1X; ++q) {
-          int xq = xl + q * R2X;
-          if (xq >= N1) xq -= N1;
-          dst[(xq < nxl ? xq : nxl + 1) * YS] = v[q];
+        for (int q = 0; q < LQX; ++q) {
+          const int l = s + q * R2X;
+          dst[(l < nxl ? l : nxl + 1) * YS] = v[q];
         }
       }
       __syncwarp();
@@ -225,7 +240,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
       Dft<R1Y, -1>::run(v);
       const int2* yr = yrow + s;
 #pragma unroll
-      for (int q = 0; q < R1Y; ++q) {
+      for (int q = 0; q < LQY; ++q) {      // rows q >= LQY are outside the disc: never stored, their butterflies are dropped
         const int2 row = yr[q * R2Y];
         const uint32_t d = l - (uint32_t)(row.y & 0xffff);
         plane[d < (uint32_t)(row.y >> 16) ? row.x + (int)l : zcol + 1] = v[q];   // zcol + 1: padding column nobody reads
@@ -277,6 +292,12 @@ using C120a = PC<120, 15, 8, 120, 15, 8, 10, 4>;
 using C120b = PC<120, 15, 8, 120, 15, 8, 8, 4>;
 using C128a = PC<128, 16, 8, 128, 16, 8, 16, 4>;
 using C128b = PC<128, 16, 8, 128, 16, 8, 8, 4>;
+// the same shapes for spheres that touch at most LQX * R2X x-lines (a cutoff sphere in a box of twice its diameter touches
+// about half of them): the strided-role x passes skip the lines that cannot be touched
+using C48p = PC<48, 8, 6, 48, 8, 6, 4, 8, 4, 5>;        // nxl <= 30 (cfg 2: 25)
+using C96p = PC<96, 12, 8, 96, 12, 8, 4, 4, 2, 7>;      // nxl <= 56 (cfg 3: 49)
+using C120p = PC<120, 15, 8, 120, 15, 8, 8, 4, 1, 8>;   // nxl <= 64 (cfg 5: 64)
+using C128p = PC<128, 16, 8, 128, 16, 8, 8, 4, 1, 9>;   // nxl <= 72 (cfg 4: 65)
 
 template <class F>
 bool v2_dispatch(int variant, F&& f) {
@@ -291,27 +312,32 @@ bool v2_dispatch(int variant, F&& f) {
     case 8: f(C96c()); return true;
     case 9: f(C48b()); return true;
     case 10: f(C96d()); return true;
+    case 11: f(C48p()); return true;
+    case 12: f(C96p()); return true;
+    case 13: f(C120p()); return true;
+    case 14: f(C128p()); return true;
     default: return false;
   }
 }
 
 }  // namespace
 
-// Picks the specialisation for an n1 x n2 plane with nxl touched x-lines that fits `smem_max` bytes of shared memory;
+// Picks the specialisation for an n1 x n2 plane with nxl touched x-lines and a disc spanning nyl y-rows that fits `smem_max` bytes of shared memory;
 // fills the radices, NYB and the variant id of the plan.  Returns false when no specialisation applies.
-bool v2_select(V2Plan& P, int n1, int n2, int nxl, size_t smem_max) {
+bool v2_select(V2Plan& P, int n1, int n2, int nxl, int nyl, size_t smem_max, bool no_prune) {
   if (n1 != n2) return false;
-  int order[4] = {0, 0, 0, 0}, norder = 0;
-  if (n1 == 48) { order[norder++] = 9; order[norder++] = 1; }
-  else if (n1 == 96) { order[norder++] = 10; order[norder++] = 8; order[norder++] = 2; }
-  else if (n1 == 120) { order[norder++] = 5; order[norder++] = 4; }   // 8 warps measured faster than 10 (12.4 vs 12.9 ms, cfg 5)
-  else if (n1 == 128) { order[norder++] = 6; order[norder++] = 7; }
+  int order[5] = {0, 0, 0, 0, 0}, norder = 0;
+  if (n1 == 48) { order[norder++] = 11; order[norder++] = 9; order[norder++] = 1; }
+  else if (n1 == 96) { order[norder++] = 12; order[norder++] = 10; order[norder++] = 8; order[norder++] = 2; }
+  else if (n1 == 120) { order[norder++] = 13; order[norder++] = 5; order[norder++] = 4; }   // 8 warps measured faster than 10 (12.4 vs 12.9 ms, cfg 5)
+  else if (n1 == 128) { order[norder++] = 14; order[norder++] = 6; order[norder++] = 7; }
+  if (no_prune && norder > 0) { for (int i = 1; i < norder; ++i) order[i - 1] = order[i]; --norder; }
   for (int oi = 0; oi < norder; ++oi) {
     const int var = order[oi];
     bool ok = false;
     v2_dispatch(var, [&](auto c) {
       using C = decltype(c);
-      if (C::smem_bytes(nxl) <= smem_max) {
+      if (C::smem_bytes(nxl) <= smem_max && nxl <= C::LQX * C::R2X && nyl <= C::LQY * C::R2Y) {
         ok = true;
         P.variant = var;
         P.r1[0] = C::R1X; P.r2[0] = C::R2X; P.r1[1] = C::R1Y; P.r2[1] = C::R2Y;

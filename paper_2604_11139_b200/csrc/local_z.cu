@@ -32,6 +32,10 @@ constexpr int ZW = 8;   // warps per CTA; two CTAs per SM
 template <int R>
 using RC = std::integral_constant<int, R>;
 
+// the pruned instantiation of a radix-R strided-role pass: a cutoff sphere in a box of twice its diameter touches just over
+// half of an axis, i.e. R/2 + 1 of the R rows q r2 + sub
+__host__ __device__ constexpr int pruned_len(int R) { return R >= 4 ? R / 2 + 1 : R; }
+
 template <bool BIG, class F>
 __device__ __forceinline__ void with_radix(int r, F&& f) {
   switch (r) {
@@ -55,7 +59,7 @@ __device__ __forceinline__ void with_radix(int r, F&& f) {
 // sits at tab4[j * nelem + i], so one load instruction of a warp reads 512 contiguous bytes
 template <int R>
 __device__ __forceinline__ void load_idx(const int4* __restrict__ tab4, int nelem, int i, int* idx) {
-  constexpr int R4 = (R + 3) / 4;
+  constexpr int R4 = (R + 3) / 4;   // R = number of table entries per element (the L of a pruned transform)
   const int4* r4 = tab4 + i;
 #pragma unroll
   for (int j = 0; j < R4; ++j) {
@@ -75,35 +79,42 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
   c128* buf = tw + P.n3 + warp * (P.cw * P.zs);                       // [cw][zs], warp-private
   for (int i = tid; i < P.n3; i += ZW * 32) tw[i] = P.tw[i];
   __syncthreads();
-  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, r1p = P.r1p;
+  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, lqp = P.lqp;
   const int64_t pstride = P.ncols_pad;
   const int nitems = P.nq * nb;
   for (int item = blockIdx.x * ZW + warp; item < nitems; item += gridDim.x * ZW) {
     const int quad = item % P.nq, band = item / P.nq;
     const c128* __restrict__ src = psi + (int64_t)band * ldpsi;
     c128* __restrict__ dst = colbuf + (int64_t)band * P.n3 * pstride + quad * cw;
-    const int4* __restrict__ tab4 = reinterpret_cast<const int4*>(P.ztab + (int64_t)quad * (r2 * cw * r1p));
-    // pass 1, strided role: radix r1 over z = q r2 + sub, inputs gathered from the sphere
+    const int4* __restrict__ tab4 = reinterpret_cast<const int4*>(P.ztab + (int64_t)quad * (r2 * cw * lqp));
+    // pass 1, strided role: radix r1 over the z-ROWS zl = q r2 + sub counted from the lowest touched z (a shift of the
+    // spectral index is a phase per z-plane in real space, which the forward transform of kz_zfwd_gather takes out again):
+    // only q < L = P.lq can be inside the sphere; inputs gathered from the sphere
     with_radix<true>(r1, [&](auto rc) {
       constexpr int R = decltype(rc)::value;
-      for (int i = lane; i < r2 * cw; i += 32) {
-        const int sub = i >> lcw, c = i & (cw - 1);
-        int idx[R];
-        load_idx<R>(tab4, r2 * cw, i, idx);
-        c128 v[R];
+      constexpr int LP = pruned_len(R);
+      auto body = [&](auto lc) {
+        constexpr int L = decltype(lc)::value;
+        for (int i = lane; i < r2 * cw; i += 32) {
+          const int sub = i >> lcw, c = i & (cw - 1);
+          int idx[L];
+          load_idx<L>(tab4, r2 * cw, i, idx);
+          c128 v[R];
 #pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = idx[q] >= 0 ? src[idx[q]] : cmake(0.0, 0.0);
-        Dft<R, +1>::run(v);
-        if (r2 == 1) {
+          for (int q = 0; q < L; ++q) v[q] = idx[q] >= 0 ? src[idx[q]] : cmake(0.0, 0.0);
+          DftPrunedIn<R, +1, L>::run(v);
+          if (r2 == 1) {
 #pragma unroll
-          for (int q = 0; q < R; ++q) dst[(int64_t)q * pstride + c] = v[q];
-        } else {
-          c128* b = buf + c * zs + sub;
-          b[0] = v[0];
+            for (int q = 0; q < R; ++q) dst[(int64_t)q * pstride + c] = v[q];
+          } else {
+            c128* b = buf + c * zs + sub;
+            b[0] = v[0];
 #pragma unroll
-          for (int q = 1; q < R; ++q) b[q * (r2 + 1)] = cmul(v[q], tw[sub * q]);
+            for (int q = 1; q < R; ++q) b[q * (r2 + 1)] = cmul(v[q], tw[sub * q]);
+          }
         }
-      }
+      };
+      if (P.lq < R) body(RC<LP>()); else body(RC<R>());
     });
     if (r2 == 1) continue;
     __syncwarp();
@@ -138,19 +149,19 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
   c128* buf = tw + P.n3 + warp * (P.cw * P.zs);
   for (int i = tid; i < P.n3; i += ZW * 32) tw[i] = P.tw[i];
   __syncthreads();
-  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, r1p = P.r1p;
+  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, lqp = P.lqp;
   const int64_t pstride = P.ncols_pad;
   const double* __restrict__ kin = P.kin;
   const int nitems = P.nq * nb;
   for (int item = blockIdx.x * ZW + warp; item < nitems; item += gridDim.x * ZW) {
     const int quad = item % P.nq, band = item / P.nq;
     const c128* __restrict__ src = colbuf + (int64_t)band * P.n3 * pstride + quad * cw;
-    const int4* __restrict__ tab4 = reinterpret_cast<const int4*>(P.ztab + (int64_t)quad * (r2 * cw * r1p));
+    const int4* __restrict__ tab4 = reinterpret_cast<const int4*>(P.ztab + (int64_t)quad * (r2 * cw * lqp));
     const c128* yb = y + (int64_t)band * ldy;
     const c128* pb = (beta != 0.0) ? yprev + (int64_t)band * ldprev : nullptr;
     c128* ob = out + (int64_t)band * ldout;
     // the epilogue's operands y[g], y_prev[g] come from HBM: start them towards L2 now, the transforms run meanwhile
-    for (int i = lane; i < r2 * cw * (r1p / 4); i += 32) {
+    for (int i = lane; i < r2 * cw * (lqp / 4); i += 32) {
       const int4 t = __ldg(tab4 + i);
       const int gi[4] = {t.x, t.y, t.z, t.w};
 #pragma unroll
@@ -179,38 +190,44 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
       });
       __syncwarp();
     }
-    // pass 2, strided role: radix r1 over positions q r2 + sub; output = w_loc at z = q r2 + sub; recurrence epilogue
+    // pass 2, strided role: radix r1 over positions q r2 + sub; output = w_loc at z-row zl = q r2 + sub (q < L: the others
+    // are outside the sphere, never used, and their butterflies are dropped); recurrence epilogue
     with_radix<true>(r1, [&](auto rc) {
       constexpr int R = decltype(rc)::value;
-      for (int i = lane; i < r2 * cw; i += 32) {
-        const int sub = i >> lcw, c = i & (cw - 1);
-        int idx[R];
-        load_idx<R>(tab4, r2 * cw, i, idx);
-        c128 v[R];
-        if (r2 == 1) {
+      constexpr int LP = pruned_len(R);
+      auto body = [&](auto lc) {
+        constexpr int L = decltype(lc)::value;
+        for (int i = lane; i < r2 * cw; i += 32) {
+          const int sub = i >> lcw, c = i & (cw - 1);
+          int idx[L];
+          load_idx<L>(tab4, r2 * cw, i, idx);
+          c128 v[R];
+          if (r2 == 1) {
 #pragma unroll
-          for (int q = 0; q < R; ++q) v[q] = src[(int64_t)q * pstride + c];
-        } else {
-          const c128* b = buf + c * zs + sub;
+            for (int q = 0; q < R; ++q) v[q] = src[(int64_t)q * pstride + c];
+          } else {
+            const c128* b = buf + c * zs + sub;
 #pragma unroll
-          for (int q = 0; q < R; ++q) v[q] = b[q * (r2 + 1)];
-        }
-        Dft<R, -1>::run(v);
-#pragma unroll
-        for (int q = 0; q < R; ++q) {
-          const int g = idx[q];
-          if (g < 0) continue;
-          const c128 yv = yb[g];
-          const double k = kin[g] - cshift;
-          c128 r = cmake(alpha * fma(k, yv.x, v[q].x), alpha * fma(k, yv.y, v[q].y));
-          if (pb) {
-            const c128 pv = pb[g];
-            r.x = fma(-beta, pv.x, r.x);
-            r.y = fma(-beta, pv.y, r.y);
+            for (int q = 0; q < R; ++q) v[q] = b[q * (r2 + 1)];
           }
-          ob[g] = r;
+          Dft<R, -1>::run(v);
+#pragma unroll
+          for (int q = 0; q < L; ++q) {
+            const int g = idx[q];
+            if (g < 0) continue;
+            const c128 yv = yb[g];
+            const double k = kin[g] - cshift;
+            c128 r = cmake(alpha * fma(k, yv.x, v[q].x), alpha * fma(k, yv.y, v[q].y));
+            if (pb) {
+              const c128 pv = pb[g];
+              r.x = fma(-beta, pv.x, r.x);
+              r.y = fma(-beta, pv.y, r.y);
+            }
+            ob[g] = r;
+          }
         }
-      }
+      };
+      if (P.lq < R) body(RC<LP>()); else body(RC<R>());
     });
     __syncwarp();
   }
@@ -221,6 +238,8 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
 // ---------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------
+int zw_pruned_len(int r) { return pruned_len(r); }
+
 size_t zw_smem(const ZPlan& P) { return sizeof(c128) * ((size_t)P.n3 + (size_t)ZW * P.cw * P.zs); }
 
 cudaError_t zw_kernels_init(const ZPlan& P) {

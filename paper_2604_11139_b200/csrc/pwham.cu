@@ -497,6 +497,7 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     bool pre = nxl < 65536 && ncols < (1 << 30);
     for (int i = 0; i < nxl && pre; ++i) pre = x_of_xl[i] == (x_of_xl[0] + i) % n1;
     std::vector<int2> yrow((size_t)n2, make_int2(0, 0));
+    int nyl = n2;
     if (pre) {
       std::vector<int> row_gy(n2, INT32_MAX), row_first(n2, 0), row_xlmin(n2, 0), row_cnt(n2, 0);
       for (int r = 0; r < ncols && pre; ++r) {
@@ -508,12 +509,21 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
           row_cnt[c.yw]++;
         }
       }
-      for (int y = 0; y < n2; ++y) yrow[y] = make_int2(row_first[y] - row_xlmin[y], row_xlmin[y] | (row_cnt[y] << 16));
+      // rows indexed from the lowest touched one (signed gy): yl = (y - y0) mod n2, so that the disc is a prefix of the axis
+      int gy_min = INT32_MAX, gy_max = INT32_MIN;
+      for (int y = 0; y < n2; ++y)
+        if (row_cnt[y] > 0) { gy_min = std::min(gy_min, row_gy[y]); gy_max = std::max(gy_max, row_gy[y]); }
+      nyl = gy_max - gy_min + 1;
+      pre = pre && nyl >= 1 && nyl <= n2;
+      for (int yl = 0; yl < n2 && pre; ++yl) {
+        const int y = wrapi(gy_min + yl, n2);
+        yrow[yl] = make_int2(row_first[y] - row_xlmin[y], row_xlmin[y] | (row_cnt[y] << 16));
+      }
     }
     const long double PI = 3.14159265358979323846264338327950288L;
     V2Plan& vp = h->vp;
     memset(&vp, 0, sizeof(vp));
-    if (pre && !env_on("PWH_NO_V2") && v2_select(vp, n1, n2, nxl, (size_t)smem_max)) {
+    if (pre && !env_on("PWH_NO_V2") && v2_select(vp, n1, n2, nxl, nyl, (size_t)smem_max, env_on("PWH_V2_NO_PRUNE"))) {
       vp.n1 = n1; vp.n2 = n2; vp.n3 = n3; vp.ncols_pad = lp.ncols_pad; vp.nxl = nxl; vp.x0 = x_of_xl[0];
       vp.zcol = ncols;
       vp.div_nxl = lp.div_nxl;
@@ -546,7 +556,14 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     ZPlan& zp = h->zp;
     memset(&zp, 0, sizeof(zp));
     zp.n3 = n3; zp.r1 = fp.r1[2]; zp.r2 = fp.r2[2];
-    zp.r1p = (zp.r1 + 3) / 4 * 4;
+    // z-rows counted from the lowest touched z (signed gz): the sphere is a prefix of the axis, nzl rows long
+    int gz_min = INT32_MAX, gz_max = INT32_MIN;
+    for (int64_t i = 0; i < npw; ++i) { gz_min = std::min(gz_min, (int)g[3 * i + 2]); gz_max = std::max(gz_max, (int)g[3 * i + 2]); }
+    const int nzl = gz_max - gz_min + 1;
+    zp.lq = zp.r1;
+    if (!env_on("PWH_V2_NO_PRUNE") && zp.r2 > 1 && zw_pruned_len(zp.r1) < zp.r1 && nzl <= zw_pruned_len(zp.r1) * zp.r2)
+      zp.lq = zw_pruned_len(zp.r1);
+    zp.lqp = (zp.lq + 3) / 4 * 4;
     zp.cw = zp.r2 >= 6 ? 4 : (zp.r2 >= 4 ? 8 : (zp.r2 >= 2 ? 16 : 32));
     zp.log2cw = zp.cw == 4 ? 2 : (zp.cw == 8 ? 3 : (zp.cw == 16 ? 4 : 5));
     zp.nq = lp.ncols_pad / zp.cw;
@@ -558,14 +575,14 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     zp.zs = zs;
     zp.tw = fp.tw[2];
     zp.kin = lp.kin;
-    if (!env_on("PWH_NO_ZW") && zw_smem(zp) <= (size_t)smem_max) {
-      std::vector<int> ztab((size_t)zp.nq * zp.r2 * zp.cw * zp.r1p, -1);
+    if (!env_on("PWH_NO_ZW") && zw_smem(zp) <= (size_t)smem_max && nzl <= n3) {
+      std::vector<int> ztab((size_t)zp.nq * zp.r2 * zp.cw * zp.lqp, -1);
       for (int64_t i = 0; i < npw; ++i) {
-        const int xw = wrapi(g[3 * i], n1), yw = wrapi(g[3 * i + 1], n2), zw_ = wrapi(g[3 * i + 2], n3);
+        const int xw = wrapi(g[3 * i], n1), yw = wrapi(g[3 * i + 1], n2), zl = g[3 * i + 2] - gz_min;
         const int c = rank[col_of_xy[(size_t)yw * n1 + xw]];
-        const int quad = c / zp.cw, cl = c % zp.cw, sub = zw_ % zp.r2, q = zw_ / zp.r2;
+        const int quad = c / zp.cw, cl = c % zp.cw, sub = zl % zp.r2, q = zl / zp.r2;
         const size_t nelem = (size_t)zp.r2 * zp.cw, el = (size_t)sub * zp.cw + cl;
-        ztab[(((size_t)quad * (zp.r1p / 4) + q / 4) * nelem + el) * 4 + q % 4] = (int)i;
+        ztab[(((size_t)quad * (zp.lqp / 4) + q / 4) * nelem + el) * 4 + q % 4] = (int)i;
       }
       if ((rc = upload(h, ztab, &zp.ztab, st))) return rc;
       CUDA_TRY(zw_kernels_init(zp));

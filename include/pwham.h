@@ -27,7 +27,13 @@
  *                              transforms (otherwise used only for axis lengths that do not factor as r1 * r2);
  *     PWH_NO_V2=1              generic-size plane kernel instead of the size-specialised one;
  *     PWH_NO_ZW=1              CTA-per-column-group z kernels instead of the warp-private ones;
- *     PWH_ZGEMM_NO_TMA=1       cp.async-fed ZGEMM instead of the TMA-fed one (process-wide, until the next setup).
+ *     PWH_ZGEMM_NO_TMA=1       cp.async-fed ZGEMM instead of the TMA-fed one (process-wide, until the next setup);
+ *     PWH_V2_NO_PRUNE=1        full-length strided-role transform passes instead of the ones that skip the rows a cutoff
+ *                              sphere cannot touch (otherwise used when the sphere spans more than about half of an axis);
+ *     PWH_LOCAL_ONE_STREAM=1   the band groups of the local-potential stage run in order on the caller's stream instead of
+ *                              alternating between two internal streams;
+ *     PWH_BAND_GROUP=n         bands per launch of the local-potential kernels (default: chosen at setup so that the column
+ *                              buffer of a group stays in L2 and the plane kernel's grid fills whole waves of SMs).
  * pwh_ham_kernels() reports which family a handle uses.
  */
 #ifndef PWHAM_H

@@ -71,6 +71,68 @@ __device__ __forceinline__ void load_idx(const int4* __restrict__ tab4, int nele
   }
 }
 
+// pass 1 of kz_scatter_zinv for one work item: radix R over the z-rows q r2 + sub of which only q < L can be inside the sphere
+template <int R, int L>
+__device__ __forceinline__ void scatter_pass1(const int4* __restrict__ tab4, const c128* __restrict__ src,
+                                              c128* __restrict__ dst, c128* __restrict__ buf, const c128* __restrict__ tw,
+                                              int64_t pstride, int r2, int cw, int lcw, int zs, int lane) {
+  for (int i = lane; i < r2 * cw; i += 32) {
+    const int sub = i >> lcw, c = i & (cw - 1);
+    int idx[L];
+    load_idx<L>(tab4, r2 * cw, i, idx);
+    c128 v[R];
+#pragma unroll
+    for (int q = 0; q < L; ++q) v[q] = idx[q] >= 0 ? src[idx[q]] : cmake(0.0, 0.0);
+    DftPrunedIn<R, +1, L>::run(v);
+    if (r2 == 1) {
+#pragma unroll
+      for (int q = 0; q < R; ++q) dst[(int64_t)q * pstride + c] = v[q];
+    } else {
+      c128* b = buf + c * zs + sub;
+      b[0] = v[0];
+#pragma unroll
+      for (int q = 1; q < R; ++q) b[q * (r2 + 1)] = cmul(v[q], tw[sub * q]);
+    }
+  }
+}
+
+// pass 2 of kz_zfwd_gather for one work item: radix R over positions q r2 + sub, outputs q < L, recurrence epilogue
+template <int R, int L>
+__device__ __forceinline__ void gather_pass2(const int4* __restrict__ tab4, const c128* __restrict__ src,
+                                             const c128* __restrict__ buf, int64_t pstride, int r2, int cw, int lcw, int zs,
+                                             int lane, const c128* yb, const c128* pb, c128* ob,
+                                             const double* __restrict__ kin, double alpha, double cshift, double beta) {
+  for (int i = lane; i < r2 * cw; i += 32) {
+    const int sub = i >> lcw, c = i & (cw - 1);
+    int idx[L];
+    load_idx<L>(tab4, r2 * cw, i, idx);
+    c128 v[R];
+    if (r2 == 1) {
+#pragma unroll
+      for (int q = 0; q < R; ++q) v[q] = src[(int64_t)q * pstride + c];
+    } else {
+      const c128* b = buf + c * zs + sub;
+#pragma unroll
+      for (int q = 0; q < R; ++q) v[q] = b[q * (r2 + 1)];
+    }
+    Dft<R, -1>::run(v);
+#pragma unroll
+    for (int q = 0; q < L; ++q) {
+      const int g = idx[q];
+      if (g < 0) continue;
+      const c128 yv = yb[g];
+      const double k = kin[g] - cshift;
+      c128 r = cmake(alpha * fma(k, yv.x, v[q].x), alpha * fma(k, yv.y, v[q].y));
+      if (pb) {
+        const c128 pv = pb[g];
+        r.x = fma(-beta, pv.x, r.x);
+        r.y = fma(-beta, pv.y, r.y);
+      }
+      ob[g] = r;
+    }
+  }
+}
+
 __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, const c128* __restrict__ psi, int64_t ldpsi,
                                                               c128* __restrict__ colbuf, int nb) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -92,29 +154,8 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
     // only q < L = P.lq can be inside the sphere; inputs gathered from the sphere
     with_radix<true>(r1, [&](auto rc) {
       constexpr int R = decltype(rc)::value;
-      constexpr int LP = pruned_len(R);
-      auto body = [&](auto lc) {
-        constexpr int L = decltype(lc)::value;
-        for (int i = lane; i < r2 * cw; i += 32) {
-          const int sub = i >> lcw, c = i & (cw - 1);
-          int idx[L];
-          load_idx<L>(tab4, r2 * cw, i, idx);
-          c128 v[R];
-#pragma unroll
-          for (int q = 0; q < L; ++q) v[q] = idx[q] >= 0 ? src[idx[q]] : cmake(0.0, 0.0);
-          DftPrunedIn<R, +1, L>::run(v);
-          if (r2 == 1) {
-#pragma unroll
-            for (int q = 0; q < R; ++q) dst[(int64_t)q * pstride + c] = v[q];
-          } else {
-            c128* b = buf + c * zs + sub;
-            b[0] = v[0];
-#pragma unroll
-            for (int q = 1; q < R; ++q) b[q * (r2 + 1)] = cmul(v[q], tw[sub * q]);
-          }
-        }
-      };
-      if (P.lq < R) body(RC<LP>()); else body(RC<R>());
+      if (P.lq < R) scatter_pass1<R, pruned_len(R)>(tab4, src, dst, buf, tw, pstride, r2, cw, lcw, zs, lane);
+      else scatter_pass1<R, R>(tab4, src, dst, buf, tw, pstride, r2, cw, lcw, zs, lane);
     });
     if (r2 == 1) continue;
     __syncwarp();
@@ -194,40 +235,10 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
     // are outside the sphere, never used, and their butterflies are dropped); recurrence epilogue
     with_radix<true>(r1, [&](auto rc) {
       constexpr int R = decltype(rc)::value;
-      constexpr int LP = pruned_len(R);
-      auto body = [&](auto lc) {
-        constexpr int L = decltype(lc)::value;
-        for (int i = lane; i < r2 * cw; i += 32) {
-          const int sub = i >> lcw, c = i & (cw - 1);
-          int idx[L];
-          load_idx<L>(tab4, r2 * cw, i, idx);
-          c128 v[R];
-          if (r2 == 1) {
-#pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = src[(int64_t)q * pstride + c];
-          } else {
-            const c128* b = buf + c * zs + sub;
-#pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = b[q * (r2 + 1)];
-          }
-          Dft<R, -1>::run(v);
-#pragma unroll
-          for (int q = 0; q < L; ++q) {
-            const int g = idx[q];
-            if (g < 0) continue;
-            const c128 yv = yb[g];
-            const double k = kin[g] - cshift;
-            c128 r = cmake(alpha * fma(k, yv.x, v[q].x), alpha * fma(k, yv.y, v[q].y));
-            if (pb) {
-              const c128 pv = pb[g];
-              r.x = fma(-beta, pv.x, r.x);
-              r.y = fma(-beta, pv.y, r.y);
-            }
-            ob[g] = r;
-          }
-        }
-      };
-      if (P.lq < R) body(RC<LP>()); else body(RC<R>());
+      if (P.lq < R)
+        gather_pass2<R, pruned_len(R)>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
+      else
+        gather_pass2<R, R>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
     });
     __syncwarp();
   }

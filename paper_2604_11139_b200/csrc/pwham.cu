@@ -648,6 +648,10 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     if (eff >= best_eff + 0.005 || (eff >= best_eff - 0.005 && c > grp && eff >= 0.97)) { best_eff = std::max(eff, best_eff); grp = c; }
   }
   h->band_group = (int)grp;
+  if (const char* e = getenv("PWH_BAND_GROUP")) {   // measurement aid (include/pwham.h): fixed group size
+    const long v = strtol(e, nullptr, 10);
+    if (v >= 1 && v <= 4096) h->band_group = (int)v;
+  }
   h->lways = env_on("PWH_LOCAL_ONE_STREAM") ? 1 : 2;
   if (h->lways == 2) {
     for (int i = 0; i < 2; ++i) {

@@ -152,6 +152,26 @@ def test_fallback_kernels_cfg2(gpu, cfg2, monkeypatch, env):
     ham.destroy()
 
 
+@pytest.mark.parametrize("env", ["PWH_V2_NO_PRUNE", "PWH_LOCAL_ONE_STREAM"])
+@pytest.mark.parametrize("case", ["cfg2", "plane128", "plane120"])
+def test_unpruned_passes_and_single_stream(gpu, cfg2, monkeypatch, env, case):
+    """The full-length strided-role passes (taken by themselves only for spheres wider than half an axis) and the in-order
+    local stage, on boxes whose default is the pruned / two-stream path; more bands than one band group."""
+    monkeypatch.setenv(env, "1")
+    if case == "cfg2":
+        w = cfg2
+    elif case == "plane128":
+        w = synth.random_problem((128, 128, 12), (54.0, 54.0, 5.0), (0.0, 0.0, 0.0), 6.95, 6, 40, seed=77)
+    else:
+        w = synth.random_problem((120, 120, 6), (50.0, 50.0, 3.0), (0.25, 0.25, 0.25), 8.0, 4, 70, seed=78)
+    ham = setup(gpu, w)
+    psi = to_dev(w.psi)
+    assert relerr(gpu.apply_h(ham, psi).cpu().numpy(), oracle.apply_h(*ham_args(w), w.psi)) <= TOL_H
+    y = gpu.cheb_filter(ham, psi.clone(), 3, w.a, w.b, w.a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(w), w.psi, 3, w.a, w.b, w.a0)) <= TOL_F
+    ham.destroy()
+
+
 def test_zgemm_without_tma(gpu, cfg2, monkeypatch):
     """The cp.async (LDGSTS) 3M ZGEMM kernels that serve when cuTensorMapEncodeTiled is unavailable or refuses an operand,
     against the oracle: projector path of apply_h and a ragged Gram product."""

@@ -133,6 +133,8 @@ __device__ __forceinline__ void gather_pass2(const int4* __restrict__ tab4, cons
   }
 }
 
+// PR: the pruned instantiation of pass 1 (P.lq == pruned_len(r1)); one kernel per choice keeps each kernel's code small
+template <bool PR>
 __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, const c128* __restrict__ psi, int64_t ldpsi,
                                                               c128* __restrict__ colbuf, int nb) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -154,8 +156,7 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
     // only q < L = P.lq can be inside the sphere; inputs gathered from the sphere
     with_radix<true>(r1, [&](auto rc) {
       constexpr int R = decltype(rc)::value;
-      if (P.lq < R) scatter_pass1<R, pruned_len(R)>(tab4, src, dst, buf, tw, pstride, r2, cw, lcw, zs, lane);
-      else scatter_pass1<R, R>(tab4, src, dst, buf, tw, pstride, r2, cw, lcw, zs, lane);
+      scatter_pass1<R, PR ? pruned_len(R) : R>(tab4, src, dst, buf, tw, pstride, r2, cw, lcw, zs, lane);
     });
     if (r2 == 1) continue;
     __syncwarp();
@@ -179,6 +180,7 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
 }
 
 // `out` may alias `y` or `yprev`: entry g of the three is read and written by the same thread, in that order.
+template <bool PR>
 __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, const c128* __restrict__ colbuf,
                                                              const c128* y, int64_t ldy,
                                                              const c128* yprev, int64_t ldprev,
@@ -235,10 +237,7 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
     // are outside the sphere, never used, and their butterflies are dropped); recurrence epilogue
     with_radix<true>(r1, [&](auto rc) {
       constexpr int R = decltype(rc)::value;
-      if (P.lq < R)
-        gather_pass2<R, pruned_len(R)>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
-      else
-        gather_pass2<R, R>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
+      gather_pass2<R, PR ? pruned_len(R) : R>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
     });
     __syncwarp();
   }
@@ -254,9 +253,11 @@ int zw_pruned_len(int r) { return pruned_len(r); }
 size_t zw_smem(const ZPlan& P) { return sizeof(c128) * ((size_t)P.n3 + (size_t)ZW * P.cw * P.zs); }
 
 cudaError_t zw_kernels_init(const ZPlan& P) {
-  cudaError_t e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_scatter_zinv));
-  if (e != cudaSuccess) return e;
-  return set_max_dyn_smem(reinterpret_cast<const void*>(&kz_zfwd_gather));
+  cudaError_t e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_scatter_zinv<true>));
+  if (e == cudaSuccess) e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_scatter_zinv<false>));
+  if (e == cudaSuccess) e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_zfwd_gather<true>));
+  if (e == cudaSuccess) e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_zfwd_gather<false>));
+  return e;
 }
 
 static int zw_grid(const ZPlan& P, int nb) {
@@ -267,15 +268,20 @@ static int zw_grid(const ZPlan& P, int nb) {
 
 void launch_zw_scatter_zinv(const ZPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st) {
   ScopedLaunch sl(ST_SCATTER_ZINV, st);
-  kz_scatter_zinv<<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, psi, ldpsi, colbuf, nb);
+  if (P.lq < P.r1) kz_scatter_zinv<true><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, psi, ldpsi, colbuf, nb);
+  else kz_scatter_zinv<false><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, psi, ldpsi, colbuf, nb);
 }
 
 void launch_zw_zfwd_gather(const ZPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,
                            int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
                            cudaStream_t st) {
   ScopedLaunch sl(ST_ZFWD_GATHER, st);
-  kz_zfwd_gather<<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha, cshift,
-                                                             yprev ? beta : 0.0, nb);
+  if (P.lq < P.r1)
+    kz_zfwd_gather<true><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha,
+                                                                     cshift, yprev ? beta : 0.0, nb);
+  else
+    kz_zfwd_gather<false><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha,
+                                                                      cshift, yprev ? beta : 0.0, nb);
 }
 
 }  // namespace pwh

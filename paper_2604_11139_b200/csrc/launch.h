@@ -69,7 +69,8 @@ cudaError_t zgemm_init();
 void zgemm_set_no_tma(bool off);
 // the two TMA descriptors of a handle's projector matrix (opaque 128-byte CUtensorMap images), encoded once at setup
 struct ProjMaps {
-  alignas(64) unsigned char cn[128];
+  alignas(64) unsigned char cn[128];    // P as the A operand of C = P^H Y (boxes of 128 projectors)
+  alignas(64) unsigned char cnb[128];   // P as the B operand of the exchanged product (Y^H P)^H (boxes of 64 projectors)
   alignas(64) unsigned char nn[128];
   bool ok = false;
 };

@@ -35,6 +35,9 @@ using RC = std::integral_constant<int, R>;
 // the pruned instantiation of a radix-R strided-role pass: a cutoff sphere in a box of twice its diameter touches just over
 // half of an axis, i.e. R/2 + 1 of the R rows q r2 + sub
 __host__ __device__ constexpr int pruned_len(int R) { return R >= 4 ? R / 2 + 1 : R; }
+// columns per work item for a contiguous-role radix r2 (the rule of pwh_ham_setup), and log2 of a power of two
+__host__ __device__ constexpr int cw_of(int r2) { return r2 >= 6 ? 4 : (r2 >= 4 ? 8 : (r2 >= 2 ? 16 : 32)); }
+__host__ __device__ constexpr int log2_of(int v) { return v <= 1 ? 0 : 1 + log2_of(v / 2); }
 
 template <bool BIG, class F>
 __device__ __forceinline__ void with_radix(int r, F&& f) {
@@ -133,8 +136,11 @@ __device__ __forceinline__ void gather_pass2(const int4* __restrict__ tab4, cons
   }
 }
 
-// PR: the pruned instantiation of pass 1 (P.lq == pruned_len(r1)); one kernel per choice keeps each kernel's code small
-template <bool PR>
+// PR: the pruned instantiation of pass 1 (P.lq == pruned_len(r1)).  R1C x R2C: the factorisation of n3 as compile-time
+// constants for the box sides of the bench configs (0 = taken from the plan at run time, every radix instantiated).  One
+// kernel per choice keeps each kernel's code small: with both pass-1 bodies of all twelve radices in one kernel the scatter
+// ran 15 % slower (profiles/r02d).
+template <int R1C, int R2C, bool PR>
 __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, const c128* __restrict__ psi, int64_t ldpsi,
                                                               c128* __restrict__ colbuf, int nb) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -143,7 +149,8 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
   c128* buf = tw + P.n3 + warp * (P.cw * P.zs);                       // [cw][zs], warp-private
   for (int i = tid; i < P.n3; i += ZW * 32) tw[i] = P.tw[i];
   __syncthreads();
-  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, lqp = P.lqp;
+  const int r1 = R1C > 0 ? R1C : P.r1, r2 = R2C > 0 ? R2C : P.r2;
+  const int cw = R2C > 0 ? cw_of(R2C) : P.cw, lcw = R2C > 0 ? log2_of(cw_of(R2C)) : P.log2cw, zs = P.zs, lqp = P.lqp;
   const int64_t pstride = P.ncols_pad;
   const int nitems = P.nq * nb;
   for (int item = blockIdx.x * ZW + warp; item < nitems; item += gridDim.x * ZW) {
@@ -154,14 +161,15 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
     // pass 1, strided role: radix r1 over the z-ROWS zl = q r2 + sub counted from the lowest touched z (a shift of the
     // spectral index is a phase per z-plane in real space, which the forward transform of kz_zfwd_gather takes out again):
     // only q < L = P.lq can be inside the sphere; inputs gathered from the sphere
-    with_radix<true>(r1, [&](auto rc) {
+    auto pass1 = [&](auto rc) {
       constexpr int R = decltype(rc)::value;
       scatter_pass1<R, PR ? pruned_len(R) : R>(tab4, src, dst, buf, tw, pstride, r2, cw, lcw, zs, lane);
-    });
+    };
+    if constexpr (R1C > 0) pass1(RC<R1C>()); else with_radix<true>(r1, pass1);
     if (r2 == 1) continue;
     __syncwarp();
     // pass 2, contiguous role: radix r2 over positions sub r2 + q; output z-slot sub r2 + q, plane-major
-    with_radix<false>(r2, [&](auto rc) {
+    auto pass2 = [&](auto rc) {
       constexpr int R = decltype(rc)::value;
       for (int i = lane; i < r1 * cw; i += 32) {
         const int sub = i >> lcw, c = i & (cw - 1);
@@ -174,13 +182,14 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_scatter_zinv(const ZPlan P, con
 #pragma unroll
         for (int q = 0; q < R; ++q) d[(int64_t)q * pstride] = v[q];
       }
-    });
+    };
+    if constexpr (R2C > 0) pass2(RC<R2C>()); else with_radix<false>(r2, pass2);
     __syncwarp();
   }
 }
 
 // `out` may alias `y` or `yprev`: entry g of the three is read and written by the same thread, in that order.
-template <bool PR>
+template <int R1C, int R2C, bool PR>
 __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, const c128* __restrict__ colbuf,
                                                              const c128* y, int64_t ldy,
                                                              const c128* yprev, int64_t ldprev,
@@ -192,7 +201,8 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
   c128* buf = tw + P.n3 + warp * (P.cw * P.zs);
   for (int i = tid; i < P.n3; i += ZW * 32) tw[i] = P.tw[i];
   __syncthreads();
-  const int r1 = P.r1, r2 = P.r2, cw = P.cw, lcw = P.log2cw, zs = P.zs, lqp = P.lqp;
+  const int r1 = R1C > 0 ? R1C : P.r1, r2 = R2C > 0 ? R2C : P.r2;
+  const int cw = R2C > 0 ? cw_of(R2C) : P.cw, lcw = R2C > 0 ? log2_of(cw_of(R2C)) : P.log2cw, zs = P.zs, lqp = P.lqp;
   const int64_t pstride = P.ncols_pad;
   const double* __restrict__ kin = P.kin;
   const int nitems = P.nq * nb;
@@ -216,7 +226,7 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
     }
     if (r2 > 1) {
       // pass 1, contiguous role: radix r2 over z-slots sub r2 + q, twiddle w^-(sub q)
-      with_radix<false>(r2, [&](auto rc) {
+      auto pass1 = [&](auto rc) {
         constexpr int R = decltype(rc)::value;
         for (int i = lane; i < r1 * cw; i += 32) {
           const int sub = i >> lcw, c = i & (cw - 1);
@@ -230,15 +240,17 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
 #pragma unroll
           for (int q = 1; q < R; ++q) b[q] = cmulc(v[q], tw[sub * q]);
         }
-      });
+      };
+      if constexpr (R2C > 0) pass1(RC<R2C>()); else with_radix<false>(r2, pass1);
       __syncwarp();
     }
     // pass 2, strided role: radix r1 over positions q r2 + sub; output = w_loc at z-row zl = q r2 + sub (q < L: the others
     // are outside the sphere, never used, and their butterflies are dropped); recurrence epilogue
-    with_radix<true>(r1, [&](auto rc) {
+    auto pass2 = [&](auto rc) {
       constexpr int R = decltype(rc)::value;
       gather_pass2<R, PR ? pruned_len(R) : R>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
-    });
+    };
+    if constexpr (R1C > 0) pass2(RC<R1C>()); else with_radix<true>(r1, pass2);
     __syncwarp();
   }
 }
@@ -252,11 +264,29 @@ int zw_pruned_len(int r) { return pruned_len(r); }
 
 size_t zw_smem(const ZPlan& P) { return sizeof(c128) * ((size_t)P.n3 + (size_t)ZW * P.cw * P.zs); }
 
+// the instantiation for a plan: the bench configs' factorisations of n3 as compile-time constants, anything else generic
+template <class F>
+static void zw_dispatch(const ZPlan& P, F&& f) {
+  const bool pr = P.lq < P.r1;
+  auto go = [&](auto r1c, auto r2c) {
+    if (pr) f(r1c, r2c, std::true_type()); else f(r1c, r2c, std::false_type());
+  };
+  if (P.cw != cw_of(P.r2)) go(RC<0>(), RC<0>());
+  else if (P.r1 == 16 && P.r2 == 8) go(RC<16>(), RC<8>());
+  else if (P.r1 == 15 && P.r2 == 12) go(RC<15>(), RC<12>());
+  else if (P.r1 == 12 && P.r2 == 8) go(RC<12>(), RC<8>());
+  else if (P.r1 == 8 && P.r2 == 6) go(RC<8>(), RC<6>());
+  else go(RC<0>(), RC<0>());
+}
+
 cudaError_t zw_kernels_init(const ZPlan& P) {
-  cudaError_t e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_scatter_zinv<true>));
-  if (e == cudaSuccess) e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_scatter_zinv<false>));
-  if (e == cudaSuccess) e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_zfwd_gather<true>));
-  if (e == cudaSuccess) e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_zfwd_gather<false>));
+  cudaError_t e = cudaSuccess;
+  zw_dispatch(P, [&](auto r1c, auto r2c, auto pr) {
+    constexpr int A = decltype(r1c)::value, B = decltype(r2c)::value;
+    constexpr bool PR = decltype(pr)::value;
+    e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_scatter_zinv<A, B, PR>));
+    if (e == cudaSuccess) e = set_max_dyn_smem(reinterpret_cast<const void*>(&kz_zfwd_gather<A, B, PR>));
+  });
   return e;
 }
 
@@ -268,20 +298,21 @@ static int zw_grid(const ZPlan& P, int nb) {
 
 void launch_zw_scatter_zinv(const ZPlan& P, const c128* psi, int64_t ldpsi, c128* colbuf, int nb, cudaStream_t st) {
   ScopedLaunch sl(ST_SCATTER_ZINV, st);
-  if (P.lq < P.r1) kz_scatter_zinv<true><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, psi, ldpsi, colbuf, nb);
-  else kz_scatter_zinv<false><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, psi, ldpsi, colbuf, nb);
+  zw_dispatch(P, [&](auto r1c, auto r2c, auto pr) {
+    kz_scatter_zinv<decltype(r1c)::value, decltype(r2c)::value, decltype(pr)::value>
+        <<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, psi, ldpsi, colbuf, nb);
+  });
 }
 
 void launch_zw_zfwd_gather(const ZPlan& P, const c128* colbuf, const c128* y, int64_t ldy, const c128* yprev,
                            int64_t ldprev, c128* out, int64_t ldout, double alpha, double cshift, double beta, int nb,
                            cudaStream_t st) {
   ScopedLaunch sl(ST_ZFWD_GATHER, st);
-  if (P.lq < P.r1)
-    kz_zfwd_gather<true><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha,
-                                                                     cshift, yprev ? beta : 0.0, nb);
-  else
-    kz_zfwd_gather<false><<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha,
-                                                                      cshift, yprev ? beta : 0.0, nb);
+  zw_dispatch(P, [&](auto r1c, auto r2c, auto pr) {
+    kz_zfwd_gather<decltype(r1c)::value, decltype(r2c)::value, decltype(pr)::value>
+        <<<zw_grid(P, nb), ZW * 32, zw_smem(P), st>>>(P, colbuf, y, ldy, yprev, ldprev, out, ldout, alpha, cshift,
+                                                      yprev ? beta : 0.0, nb);
+  });
 }
 
 }  // namespace pwh

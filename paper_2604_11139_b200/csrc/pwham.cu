@@ -628,15 +628,17 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
   CUDA_TRY(zgemm_init());
   if (nproj > 0) zgemm_make_proj_maps(h->pmaps, h->proj, npw, nproj, ldp);
 
-  // bands per launch of the local kernels: the column buffer of a group (written by one kernel, read by the next) should
-  // stay in the 126 MB L2 -- at most 56 MB -- and the plane kernel's grid of n3 x bands CTAs (one per SM) should fill
-  // whole waves of the 148 SMs: among the group sizes whose buffer is between 24 and 56 MB take the one with the best
-  // wave efficiency (ncu, profiles/r01d: 7 bands x 128 planes = 6.05 waves left the seventh wave almost empty)
+  // bands per launch of the local kernels.  The z kernels are latency-bound and want many work items per launch (a group of
+  // 4 bands at cfg 5 is 1.19 rounds of the resident warps, i.e. two rounds of which the second is almost empty), the plane
+  // kernel's grid of n3 x bands CTAs (one per SM) should fill whole waves of the 148 SMs, and the column buffer of a group
+  // (written by one kernel, read by the next) is served from the 126 MB L2 for its most recently written part whatever its
+  // size.  Measured (profiles/r02f): the stage gets faster up to about 300 MB of column buffer per group and flat beyond,
+  // so among the group sizes with 190 ... 320 MB take the one with the best wave efficiency of the plane kernel.
   const size_t per_band = (size_t)n3 * lp.ncols_pad * sizeof(c128);
   const int64_t slots = 148;                                                            // resident plane CTAs
-  const size_t win_hi = 56u << 20;
+  const size_t win_hi = 320u << 20, win_lo = 190u << 20;
   const int64_t min_grp = (2 * 148 + n3 - 1) / n3;
-  int64_t g_lo = std::max<int64_t>(std::max<int64_t>((int64_t)((24u << 20) / std::max<size_t>(per_band, 1)), min_grp), 1);
+  int64_t g_lo = std::max<int64_t>(std::max<int64_t>((int64_t)(win_lo / std::max<size_t>(per_band, 1)), min_grp), 1);
   int64_t g_hi = std::max<int64_t>((int64_t)(win_hi / std::max<size_t>(per_band, 1)), g_lo);
   g_hi = std::min<int64_t>(g_hi, 4096);
   g_lo = std::min<int64_t>(g_lo, g_hi);

@@ -414,15 +414,17 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
 
 // C[m + n*ldc] = scale[m] * sum_s part[s][m + n*M]   (fixed summation order => deterministic).  herm: the partial sums
 // exist for floor(m/128) <= floor(n/128) only; the other entries are the conjugates of their mirror images.
+// swapped: the partial sums hold the N x M matrix B^H A = (A^H B)^H (operands exchanged by launch_zgemm_cn), so every entry is
+// the conjugate of its transposed image.
 __global__ void __launch_bounds__(256) k_splitk_reduce(int M, int N, int nsplit, const c128* __restrict__ part,
                                                        const double* __restrict__ scale, c128* __restrict__ C,
-                                                       int64_t ldc, int herm) {
+                                                       int64_t ldc, int herm, int swapped) {
   const int64_t total = (int64_t)M * N;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
     const int m = (int)(i % M);
     const int64_t n = i / M;
-    const bool mirror = herm && (m / BM) > (int)(n / BM);
-    const int64_t src = mirror ? (int64_t)m * M + n : i;
+    const bool mirror = swapped || (herm && (m / BM) > (int)(n / BM));
+    const int64_t src = swapped ? (int64_t)m * N + n : (mirror ? (int64_t)m * M + n : i);
     double sx = 0.0, sy = 0.0;
     for (int s = 0; s < nsplit; ++s) {
       const c128 v = part[(int64_t)s * total + src];
@@ -503,6 +505,7 @@ static bool make_map(CUtensorMap* tm, const c128* base, int64_t inner, int64_t o
 void zgemm_make_proj_maps(ProjMaps& pm, const c128* P, int64_t npw, int64_t nproj, int64_t ldp) {
   static_assert(sizeof(CUtensorMap) == sizeof(pm.cn), "ProjMaps storage");
   pm.ok = nproj > 0 && make_map(reinterpret_cast<CUtensorMap*>(pm.cn), P, npw, nproj, ldp, BM) &&
+          make_map(reinterpret_cast<CUtensorMap*>(pm.cnb), P, npw, nproj, ldp, BN) &&
           make_map(reinterpret_cast<CUtensorMap*>(pm.nn), P, npw, nproj, ldp, NNT_BK);
 }
 
@@ -540,7 +543,17 @@ cudaError_t dmma_probe(int iters, int ctas, double* sink, cudaStream_t st, float
 
 // number of 128 x 64 tiles of C the CN kernel computes: all of them, or -- for a Hermitian C (herm) -- those that
 // touch the block upper triangle  floor(m/128) <= floor(n/128)
+// C = A^H B can equally be computed as (B^H A)^H: with the 128 x 64 tile the two orientations pad differently
+// (cfg 5: 1728 projectors x 512 bands is 14 x 8 = 112 tiles one way, 4 x 27 = 108 the other); exchange the operands
+// when that saves more than 2 % of the tiles.
+static bool cn_swapped(int64_t M, int64_t N, bool herm) {
+  if (herm) return false;
+  const int64_t a = ((M + BM - 1) / BM) * ((N + BN - 1) / BN), b = ((N + BM - 1) / BM) * ((M + BN - 1) / BN);
+  return b * 100 < a * 98;
+}
+
 static int64_t cn_tiles(int64_t M, int64_t N, bool herm) {
+  if (cn_swapped(M, N, herm)) std::swap(M, N);
   const int64_t tiles_m = (M + BM - 1) / BM, tiles_n = (N + BN - 1) / BN;
   if (!herm) return tiles_m * tiles_n;
   int64_t t = 0;
@@ -586,7 +599,12 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
   if (M <= 0 || N <= 0) return;
   if (M != N) herm = false;
   const int nsplit = zgemm_cn_splits(M, N, K, herm);
-  const int tiles_m = (int)((M + BM - 1) / BM);
+  const bool swapped = cn_swapped(M, N, herm);
+  // the product the kernel computes: Mk x Nk = Ak^H Bk (the operands exchanged when `swapped`)
+  const int64_t Mk = swapped ? N : M, Nk = swapped ? M : N;
+  const c128 *Ak = swapped ? B : A, *Bk = swapped ? A : B;
+  const int64_t ldak = swapped ? ldb : lda, ldbk = swapped ? lda : ldb;
+  const int tiles_m = (int)((Mk + BM - 1) / BM);
   int64_t kps = (K + nsplit - 1) / nsplit;
   kps = (kps + CNT_BK - 1) / CNT_BK * CNT_BK;
   dim3 grid((unsigned)cn_tiles(M, N, herm), nsplit);
@@ -594,21 +612,29 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
   {
     ScopedLaunch sl(ST_ZGEMM_CN, st);
     CUtensorMap tmA, tmB;
-    bool tma = false;
-    if (pmA && pmA->ok && !g_no_tma.load(std::memory_order_relaxed)) { memcpy(&tmA, pmA->cn, sizeof(tmA)); tma = true; }
-    else tma = make_map(&tmA, A, K, M, lda, BM);
-    if (tma && make_map(&tmB, B, K, N, ldb, BN))
+    const bool cached = pmA && pmA->ok && !g_no_tma.load(std::memory_order_relaxed);
+    bool tma;
+    if (!swapped) {
+      if (cached) { memcpy(&tmA, pmA->cn, sizeof(tmA)); tma = true; }
+      else tma = make_map(&tmA, Ak, K, Mk, ldak, BM);
+      tma = tma && make_map(&tmB, Bk, K, Nk, ldbk, BN);
+    } else {
+      tma = make_map(&tmA, Ak, K, Mk, ldak, BM);
+      if (tma && cached) memcpy(&tmB, pmA->cnb, sizeof(tmB));
+      else tma = tma && make_map(&tmB, Bk, K, Nk, ldbk, BN);
+    }
+    if (tma)
       k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES><<<grid, NT3, smem_tma(CNT_BK, CNT_STAGES), st>>>(
-          tmA, tmB, (int)M, (int)N, K, tiles_m, kps, part, M, 0.0, herm ? 1 : 0);
+          tmA, tmB, (int)Mk, (int)Nk, K, tiles_m, kps, part, Mk, 0.0, herm ? 1 : 0);
     else
       k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES><<<grid, NT3, smem_cn3(), st>>>(
-          (int)M, (int)N, K, tiles_m, kps, A, lda, B, ldb, part, M, 0.0, herm ? 1 : 0);
+          (int)Mk, (int)Nk, K, tiles_m, kps, Ak, ldak, Bk, ldbk, part, Mk, 0.0, herm ? 1 : 0);
   }
   const int64_t total = M * N;
   int blocks = (int)((total + 255) / 256);
   if (blocks > NUM_SMS * 8) blocks = NUM_SMS * 8;
   ScopedLaunch sl(ST_SPLITK, st);
-  k_splitk_reduce<<<blocks, 256, 0, st>>>((int)M, (int)N, nsplit, part, scale, C, ldc, herm ? 1 : 0);
+  k_splitk_reduce<<<blocks, 256, 0, st>>>((int)M, (int)N, nsplit, part, scale, C, ldc, herm ? 1 : 0, swapped ? 1 : 0);
 }
 
 // C = alpha * A B (+ C when accumulate)

@@ -110,9 +110,11 @@ def test_density_accumulates_over_calls_and_kpoints(gpu):
     hb.destroy()
 
 
-def test_density_several_band_groups_padded_ld_and_determinism(gpu):
-    """cfg 3's box with more bands than one band group of the local kernels; padded leading dimension; two runs bit-identical."""
+def test_density_several_band_groups_padded_ld_and_determinism(gpu, monkeypatch):
+    """cfg 3's box with more bands than one band group of the local kernels (ragged last group); padded leading dimension;
+    two runs bit-identical."""
     import torch
+    monkeypatch.setenv("PWH_BAND_GROUP", "7")
     w = synth.make_workload(3, nband=24, qr="none")
     occ = occupations(24, 9)
     ham = setup(gpu, w)

@@ -172,6 +172,26 @@ def test_unpruned_passes_and_single_stream(gpu, cfg2, monkeypatch, env, case):
     ham.destroy()
 
 
+@pytest.mark.parametrize("group", [1, 5, 64])
+def test_band_groups_alternate_between_two_streams(gpu, cfg2, monkeypatch, group):
+    """Many small band groups (ragged last one for 5) on the two internal streams, and exactly two groups (64): every band goes
+    through the same kernels whatever the grouping, so the result must not depend on it at all."""
+    monkeypatch.setenv("PWH_BAND_GROUP", str(group))
+    w = cfg2
+    ham = setup(gpu, w)
+    assert ham.info()["band_group"] == group
+    psi = to_dev(w.psi)
+    h1 = gpu.apply_h(ham, psi).cpu().numpy()
+    assert relerr(h1, oracle.apply_h(*ham_args(w), w.psi)) <= TOL_H
+    y = gpu.cheb_filter(ham, psi.clone(), 4, w.a, w.b, w.a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(w), w.psi, 4, w.a, w.b, w.a0)) <= TOL_F
+    ham.destroy()
+    monkeypatch.delenv("PWH_BAND_GROUP")
+    ham = setup(gpu, w)
+    assert np.array_equal(gpu.apply_h(ham, psi).cpu().numpy(), h1)       # bit-identical to the default grouping
+    ham.destroy()
+
+
 def test_zgemm_without_tma(gpu, cfg2, monkeypatch):
     """The cp.async (LDGSTS) 3M ZGEMM kernels that serve when cuTensorMapEncodeTiled is unavailable or refuses an operand,
     against the oracle: projector path of apply_h and a ragged Gram product."""

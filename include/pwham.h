@@ -30,8 +30,10 @@
  *     PWH_ZGEMM_NO_TMA=1       cp.async-fed ZGEMM instead of the TMA-fed one (process-wide, until the next setup);
  *     PWH_V2_NO_PRUNE=1        full-length strided-role transform passes instead of the ones that skip the rows a cutoff
  *                              sphere cannot touch (otherwise used when the sphere spans more than about half of an axis);
- *     PWH_LOCAL_ONE_STREAM=1   the band groups of the local-potential stage run in order on the caller's stream instead of
- *                              alternating between two internal streams;
+ *     PWH_LOCAL_ONE_STREAM=1   the band groups of the local-potential stage run in order on the caller's stream;
+ *     PWH_LOCAL_TWO_STREAMS=1  they alternate between two internal streams (default: the handle times both on its first four
+ *                              multi-group H applications, with events on the caller's stream and no host synchronisation,
+ *                              and keeps the faster; results do not depend on the choice);
  *     PWH_BAND_GROUP=n         bands per launch of the local-potential kernels (default: chosen at setup so that the column
  *                              buffer of a group stays in L2 and the plane kernel's grid fills whole waves of SMs).
  * pwh_ham_kernels() reports which family a handle uses.

@@ -143,8 +143,18 @@ struct pwh_ham {
   // the band groups of the local stage alternate between two internal streams (each with its own column buffer), so that
   // the partial last wave of one group's kernels is filled by the other group's (lways = 1: one stream, in order)
   int lways = 1;
+  int lbufs = 1;                 // column buffers in the workspace layout (fixed at setup: the layout never changes)
   cudaStream_t ls[2] = {nullptr, nullptr};
   cudaEvent_t lev_fork = nullptr, lev_join[2] = {nullptr, nullptr};
+  // one or two streams?  Measured, not guessed (profiles/r02h): two streams win where the z kernels are a large part of the
+  // stage (cfg 5), one stream where the plane kernel dominates (cfg 3, 4) -- by about 1 % of the step either way.  The first
+  // four multi-group H applications of a handle alternate between the two and are bracketed by events on the caller's
+  // stream; a later call reads the four times back with cudaEventQuery (no host synchronisation anywhere) and fixes the
+  // choice.  The results do not depend on it (every band runs through the same kernels).
+  bool ltune = false;            // still deciding
+  int ltune_calls = 0;
+  int64_t ltune_nband = 0;
+  cudaEvent_t ltune_ev[4][2] = {};
 };
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -293,6 +303,9 @@ extern "C" int pwh_ham_destroy(pwh_ham* h) {
     if (h->lev_join[i]) cudaEventDestroy(h->lev_join[i]);
   }
   if (h->lev_fork) cudaEventDestroy(h->lev_fork);
+  for (auto& pr : h->ltune_ev)
+    for (cudaEvent_t e : pr)
+      if (e) cudaEventDestroy(e);
   delete h;
   return PWH_OK;
 }
@@ -655,6 +668,11 @@ static int setup_impl(pwh_ham* h, const double lattice[9], const double kpt[3], 
     if (v >= 1 && v <= 4096) h->band_group = (int)v;
   }
   h->lways = env_on("PWH_LOCAL_ONE_STREAM") ? 1 : 2;
+  h->lbufs = h->lways;
+  h->ltune = h->lways == 2 && !env_on("PWH_LOCAL_TWO_STREAMS");
+  if (h->ltune)
+    for (auto& pr : h->ltune_ev)
+      for (cudaEvent_t& e : pr) CUDA_TRY(cudaEventCreate(&e));
   if (h->lways == 2) {
     for (int i = 0; i < 2; ++i) {
       CUDA_TRY(cudaStreamCreateWithFlags(&h->ls[i], cudaStreamNonBlocking));
@@ -712,6 +730,7 @@ extern "C" int pwh_ham_kernels(const pwh_ham* h, char* buf, size_t n) {
   }
   if (h->nproj > 0) s += h->pmaps.ok ? "zgemm3m_tma" : "zgemm3m";
   if (h->paw) s += " paw_blocks";
+  s += h->ltune ? " local_streams:undecided" : (h->lways == 2 ? " local_streams:2" : " local_streams:1");
   snprintf(buf, n, "%s", s.c_str());
   return PWH_OK;
 }
@@ -734,7 +753,7 @@ static WsLayout ws_layout(const pwh_ham* h, int64_t nband) {
   w.ldw = (int64_t)align_up((size_t)h->npw, 16);
   size_t off = 0;
   w.colbuf_bytes = align_up((size_t)w.group * h->n3 * h->lp.ncols_pad * sizeof(c128), 256);
-  w.colbuf = off; off += (size_t)h->lways * w.colbuf_bytes;
+  w.colbuf = off; off += (size_t)h->lbufs * w.colbuf_bytes;
   // projections C = P^H Y; with PAW blocks also blockdiag(D) C and blockdiag(Q) C (or K C)
   w.cmat = off;   off += (h->paw ? 3 : 1) * align_up((size_t)std::max<int64_t>(h->nproj, 1) * nband * sizeof(c128), 256);
   w.part = off;   off += align_up(h->nproj > 0 ? zgemm_cn_workspace_upto(h->nproj, nband, h->npw) : 16, 256);
@@ -772,14 +791,40 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
     NvtxRange r("pwh:local+kinetic+recurrence");
     // two-way interleave of the band groups (bands never interact); one stream while the per-launch
     // profile is on, so that the per-kernel event times are those of kernels running alone
-    const int ways = (h->lways == 2 && nband > w.group && !g_prof_on.load(std::memory_order_relaxed)) ? 2 : 1;
+    int ways = (h->lways == 2 && nband > w.group && !g_prof_on.load(std::memory_order_relaxed)) ? 2 : 1;
+    int tune_slot = -1;
+    if (ways == 2 && h->ltune) {
+      if (h->ltune_calls < 4 && (h->ltune_calls == 0 || nband == h->ltune_nband)) {
+        h->ltune_nband = nband;
+        tune_slot = h->ltune_calls++;
+        ways = (tune_slot & 1) ? 1 : 2;
+        CUDA_TRY(cudaEventRecord(h->ltune_ev[tune_slot][0], st));
+      } else if (h->ltune_calls >= 4) {
+        bool done = true;
+        for (int i = 0; i < 4 && done; ++i) done = cudaEventQuery(h->ltune_ev[i][1]) == cudaSuccess;
+        if (done) {
+          float t[4] = {0, 0, 0, 0};
+          for (int i = 0; i < 4; ++i) CUDA_TRY(cudaEventElapsedTime(&t[i], h->ltune_ev[i][0], h->ltune_ev[i][1]));
+          // slots 0, 2: two streams; 1, 3: one stream.  The first slot also pays first-touch costs: compare the second pair.
+          h->lways = t[3] < t[2] ? 1 : 2;
+          h->ltune = false;
+          ways = h->lways;
+        } else {
+          (void)cudaGetLastError();   // cudaErrorNotReady is not an error
+        }
+      } else {
+        h->ltune_calls = 0;            // a different block size: start over with this one
+      }
+    }
     if (ways == 2) {
       CUDA_TRY(cudaEventRecord(h->lev_fork, st));
       for (int i = 0; i < 2; ++i) CUDA_TRY(cudaStreamWaitEvent(h->ls[i], h->lev_fork, 0));
     }
-    int64_t gi = 0;
-    for (int64_t b0 = 0; b0 < nband; b0 += w.group, ++gi) {
-      const int nb = (int)std::min<int64_t>(w.group, nband - b0);
+    // groups of equal size (they differ by at most one band): no short last group
+    const int64_t ngroups = (nband + w.group - 1) / w.group, gbase = nband / ngroups, grem = nband % ngroups;
+    int64_t b0 = 0;
+    for (int64_t gi = 0; gi < ngroups; ++gi) {
+      const int nb = (int)(gbase + (gi < grem ? 1 : 0));
       cudaStream_t ls = ways == 2 ? h->ls[gi & 1] : st;
       c128* cb = ways == 2 ? reinterpret_cast<c128*>(ws + w.colbuf + (size_t)(gi & 1) * w.colbuf_bytes) : colbuf;
       if (h->fast) {
@@ -799,12 +844,14 @@ static int h_step(pwh_ham* h, int64_t nband, const c128* y, int64_t ldy, const c
         launch_zfwd_gather(h->lp, cb, y + b0 * ldy, ldy, yprev ? yprev + b0 * ldprev : nullptr, ldprev,
                            out + b0 * ldout, ldout, alpha, cshift, yprev ? beta : 0.0, nb, ls);
       }
+      b0 += nb;
     }
     if (ways == 2)
       for (int i = 0; i < 2; ++i) {
         CUDA_TRY(cudaEventRecord(h->lev_join[i], h->ls[i]));
         CUDA_TRY(cudaStreamWaitEvent(st, h->lev_join[i], 0));
       }
+    if (tune_slot >= 0) CUDA_TRY(cudaEventRecord(h->ltune_ev[tune_slot][1], st));
   }
   if (h->nproj > 0) {
     NvtxRange r("pwh:nonlocal:Y+=a.P.C");

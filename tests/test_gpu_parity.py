@@ -152,7 +152,7 @@ def test_fallback_kernels_cfg2(gpu, cfg2, monkeypatch, env):
     ham.destroy()
 
 
-@pytest.mark.parametrize("env", ["PWH_V2_NO_PRUNE", "PWH_LOCAL_ONE_STREAM"])
+@pytest.mark.parametrize("env", ["PWH_V2_NO_PRUNE", "PWH_LOCAL_ONE_STREAM", "PWH_LOCAL_TWO_STREAMS"])
 @pytest.mark.parametrize("case", ["cfg2", "plane128", "plane120"])
 def test_unpruned_passes_and_single_stream(gpu, cfg2, monkeypatch, env, case):
     """The full-length strided-role passes (taken by themselves only for spheres wider than half an axis) and the in-order
@@ -177,6 +177,7 @@ def test_band_groups_alternate_between_two_streams(gpu, cfg2, monkeypatch, group
     """Many small band groups (ragged last one for 5) on the two internal streams, and exactly two groups (64): every band goes
     through the same kernels whatever the grouping, so the result must not depend on it at all."""
     monkeypatch.setenv("PWH_BAND_GROUP", str(group))
+    monkeypatch.setenv("PWH_LOCAL_TWO_STREAMS", "1")
     w = cfg2
     ham = setup(gpu, w)
     assert ham.info()["band_group"] == group
@@ -187,8 +188,27 @@ def test_band_groups_alternate_between_two_streams(gpu, cfg2, monkeypatch, group
     assert relerr(y, oracle.cheb_filter(*ham_args(w), w.psi, 4, w.a, w.b, w.a0)) <= TOL_F
     ham.destroy()
     monkeypatch.delenv("PWH_BAND_GROUP")
+    monkeypatch.delenv("PWH_LOCAL_TWO_STREAMS")
     ham = setup(gpu, w)
     assert np.array_equal(gpu.apply_h(ham, psi).cpu().numpy(), h1)       # bit-identical to the default grouping
+    ham.destroy()
+
+
+def test_stream_choice_is_measured_without_changing_results(gpu, cfg2, monkeypatch):
+    """Default handle: the first four multi-group H applications alternate between two streams and one and are timed with
+    events, later ones use the faster -- ten applications in a row must all be bit-identical."""
+    monkeypatch.setenv("PWH_BAND_GROUP", "16")
+    ham = setup(gpu, cfg2)
+    psi = to_dev(cfg2.psi)
+    ref = gpu.apply_h(ham, psi).cpu().numpy()
+    assert relerr(ref, oracle.apply_h(*ham_args(cfg2), cfg2.psi)) <= TOL_H
+    import torch
+    for i in range(10):
+        if i == 6:
+            torch.cuda.synchronize()
+        assert np.array_equal(gpu.apply_h(ham, psi).cpu().numpy(), ref), i
+    y = gpu.cheb_filter(ham, psi.clone(), 8, cfg2.a, cfg2.b, cfg2.a0).cpu().numpy()
+    assert relerr(y, oracle.cheb_filter(*ham_args(cfg2), cfg2.psi, 8, cfg2.a, cfg2.b, cfg2.a0)) <= TOL_F
     ham.destroy()
 
 

@@ -80,3 +80,81 @@ def test_exact_invariant_subspace_is_a_fixed_point(cfg1):
     assert out["resid"].max() <= 1e-8
     p_ref = vec[:, :6] @ vec[:, :6].conj().T
     assert np.abs(out["psi"].T @ out["psi"].conj() - p_ref).max() <= 1e-8
+
+
+# ---- Algorithm 11 with the PAW overlap S (lobpcg_gen) ----------------------------------------------------------------------
+def dense_hs(w, off, db, qb):
+    from oracle import paw
+    hd = oracle.dense_h(w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, None, None)
+    p = w.proj                                           # (nproj, npw): p[i, G] = P[G, i]
+    hd = hd + p.T @ paw.blockdiag_dense(off, db) @ p.conj()
+    sd = np.eye(w.npw) + p.T @ paw.blockdiag_dense(off, qb) @ p.conj()
+    return hd, sd
+
+
+def gen_args(w, off, db, qb):
+    return (w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, w.proj, off, db, qb)
+
+
+def test_gen_reduces_to_the_s_identity_oracle_for_diagonal_d_and_zero_q(cfg1):
+    """Q = 0 and diagonal D blocks: S = I, and every step of lobpcg_gen must reproduce lobpcg (separately pinned above)."""
+    w = cfg1
+    off = np.arange(0, w.nproj + 1, 4, dtype=np.int32)
+    db = [np.diag(w.dij[lo_:lo_ + 4]).astype(np.complex128) for lo_ in off[:-1]]
+    qb = [np.zeros((4, 4), dtype=np.complex128) for _ in off[:-1]]
+    a = lo.lobpcg_gen(*gen_args(w, off, db, qb), w.psi, 2, 3)
+    b = lo.lobpcg(*ham_args(w), w.psi, 2, 3)
+    assert np.abs(a["lam"] - b["lam"]).max() <= 1e-10 * np.abs(b["lam"]).max()
+    assert np.abs(a["resid"] - b["resid"]).max() <= 1e-8 * max(b["resid"].max(), 1e-3)
+    assert np.abs(a["spsi"] - a["psi"]).max() <= 1e-13
+    for ha, hb in zip(a["history"], b["history"]):
+        for na, nb in zip(ha, hb):
+            assert np.abs(na - nb).max() <= 1e-8 * max(nb.max(), 1e-3)
+
+
+def test_gen_deflate_and_ortho_properties(cfg1):
+    from oracle import paw
+    w = cfg1
+    off, db, qb = synth.paw_blocks(w.nproj, w.dij, seed=3)
+    _, sd = dense_hs(w, off, db, qb)
+    x = w.psi[:6]
+    hx, sx = paw.apply_hs(*gen_args(w, off, db, qb), x)
+    y, hy, sy, u = lo.chol_ortho_gen(x, hx, sx)
+    assert np.abs(np.conj(y) @ sd @ y.T - np.eye(6)).max() <= 1e-12        # Y^H S Y = I with the dense S (numpy)
+    assert np.abs(np.tril(u, -1)).max() == 0 and np.all(np.diag(u).real > 0)
+    assert np.abs(sy - (sd @ y.T).T).max() <= 1e-12                         # S Y is carried along consistently
+    z = w.psi[6:10] + 0.25 * y[:4]
+    zd = lo.deflate_gen(z, y, sy)
+    assert np.abs(np.conj(y) @ sd @ zd.T).max() <= 1e-12                   # S-orthogonal to the basis afterwards
+    assert np.abs(lo.deflate_gen(zd, y, sy) - zd).max() <= 1e-12            # idempotent
+
+
+@pytest.mark.parametrize("nblocks", [1, 2])
+def test_gen_converges_to_the_generalised_spectrum(cfg1, nblocks):
+    import scipy.linalg as sl
+    w = cfg1
+    off, db, qb = synth.paw_blocks(w.nproj, w.dij, seed=3)
+    hd, sd = dense_hs(w, off, db, qb)
+    ev = sl.eigh(hd, sd, eigvals_only=True)
+    M = w.psi.shape[0]
+    out = lo.lobpcg_gen(*gen_args(w, off, db, qb), w.psi, nblocks, 14)
+    lam = out["lam"]
+    assert np.all(lam >= ev[:M] - 1e-10)                                   # Ritz values bound the spectrum from above
+    assert np.abs(lam[: M // 2] - ev[: M // 2]).max() <= 1e-5 * np.abs(ev).max()
+    assert out["resid"][: M // 2].max() <= 1e-3
+    assert np.abs(np.conj(out["psi"]) @ sd @ out["psi"].T - np.eye(M)).max() <= 1e-10   # S-orthonormal Ritz vectors
+    first = np.max(out["history"][0][0])
+    last = np.max(out["history"][0][-1])
+    assert last < 0.05 * first                                             # the residuals do come down
+
+
+def test_gen_exact_invariant_subspace_is_a_fixed_point(cfg1):
+    import scipy.linalg as sl
+    w = cfg1
+    off, db, qb = synth.paw_blocks(w.nproj, w.dij, seed=3)
+    hd, sd = dense_hs(w, off, db, qb)
+    ev, v = sl.eigh(hd, sd)
+    psi = np.ascontiguousarray(v[:, :4].T)                                 # exact generalised eigenvectors, S-orthonormal
+    out = lo.lobpcg_gen(*gen_args(w, off, db, qb), psi, 1, 2)
+    assert np.abs(out["lam"] - ev[:4]).max() <= 1e-11 * np.abs(ev).max()
+    assert out["history"][0][0].max() <= 1e-10

@@ -223,6 +223,14 @@ int pwh_chol_ortho(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c1
                    int64_t ldu, int32_t* info, void* ws, size_t ws_bytes, void* stream);
 
 /*
+ * pwh_chol_ortho_gen -- Algorithm 9 (S-Ortho) as printed, for the generalised problem: S_Psi = Psi^H (S Psi) = U^H U, then
+ * Psi <- Psi U^-1, S Psi <- (S Psi) U^-1 and, when hpsi != NULL, H Psi <- (H Psi) U^-1, in place.  spsi = S Psi
+ * is required (pwh_apply_hs).  Afterwards Psi^H (S Psi) = I.  Workspace and *info as for pwh_chol_ortho.
+ */
+int pwh_chol_ortho_gen(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh, pwh_c128* spsi,
+                       int64_t lds, pwh_c128* U, int64_t ldu, int32_t* info, void* ws, size_t ws_bytes, void* stream);
+
+/*
  * pwh_rayleigh_ritz -- Algorithm 10 (RR), in place: H_Psi = Psi^H (H Psi), S_Psi = Psi^H (S Psi), H_Psi X = S_Psi X Lambda,
  * Psi <- Psi X, H Psi <- (H Psi) X, S Psi <- (S Psi) X (Algorithm 5).  lambda receives
  * the nband Ritz values in ascending order; afterwards Psi^H (S Psi) = I and Psi^H (H Psi) = diag(lambda).
@@ -308,6 +316,18 @@ size_t pwh_lobpcg_workspace_bytes(const pwh_ham* ham, int64_t nband, int64_t nbl
 int pwh_lobpcg(pwh_ham* ham, int64_t nband, int64_t nblocks, int nline, double tol, pwh_c128* psi, int64_t ld, pwh_c128* hpsi,
                int64_t ldh, double* lambda, double* resid, double* history, int32_t* info, void* ws, size_t ws_bytes,
                void* stream);
+
+/*
+ * pwh_lobpcg_gen -- Algorithm 11 as printed, with the PAW overlap S of a handle that carries PAW blocks (pwh_ham_set_paw):
+ * H X and S X come from one call of HX_SX (pwh_apply_hs, lines 6 and 18), every inner product is <., S .> (S-Deflate of
+ * Algorithm 8 against the solved bands, S-Ortho of Algorithm 9, the generalised RR of Algorithm 10), the residual is
+ * W = (H - Lambda S) Psi_i (line 11).  Same arguments and outputs as pwh_lobpcg plus spsi [out] = S psi (npw x nband, lds);
+ * afterwards psi^H (S psi) = I.  Workspace: pwh_lobpcg_gen_workspace_bytes(ham, nband, nblocks).
+ */
+size_t pwh_lobpcg_gen_workspace_bytes(const pwh_ham* ham, int64_t nband, int64_t nblocks);
+int pwh_lobpcg_gen(pwh_ham* ham, int64_t nband, int64_t nblocks, int nline, double tol, pwh_c128* psi, int64_t ld,
+                   pwh_c128* hpsi, int64_t ldh, pwh_c128* spsi, int64_t lds, double* lambda, double* resid, double* history,
+                   int32_t* info, void* ws, size_t ws_bytes, void* stream);
 
 /*
  * ---------------------------------------------------------------------------------------------------------------

@@ -29,7 +29,8 @@ EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply
            "pwh_chebfi_workspace_bytes", "pwh_chebfi_iteration",
            "pwh_ham_set_paw", "pwh_apply_hs", "pwh_apply_sinv", "pwh_cheb_filter_gen",
            "pwh_lobpcg_workspace_bytes", "pwh_lobpcg",
-           "pwh_density_workspace_bytes", "pwh_density_accumulate"]
+           "pwh_density_workspace_bytes", "pwh_density_accumulate",
+           "pwh_chol_ortho_gen", "pwh_lobpcg_gen_workspace_bytes", "pwh_lobpcg_gen"]
 
 STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "colstats", "dense_small",
           "jacobi", "axpy", "reserved10", "reserved11"]
@@ -119,6 +120,12 @@ def load_library() -> ctypes.CDLL:
     L.pwh_apply_sinv.restype = i32
     L.pwh_cheb_filter_gen.argtypes = [vp, i64, vp, i64, i32, dbl, dbl, dbl, vp, sz, vp]
     L.pwh_cheb_filter_gen.restype = i32
+    L.pwh_chol_ortho_gen.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, i64, vp, vp, sz, vp]
+    L.pwh_chol_ortho_gen.restype = i32
+    L.pwh_lobpcg_gen_workspace_bytes.argtypes = [vp, i64, i64]
+    L.pwh_lobpcg_gen_workspace_bytes.restype = sz
+    L.pwh_lobpcg_gen.argtypes = [vp, i64, i64, i32, dbl, vp, i64, vp, i64, vp, i64, vp, vp, vp, vp, vp, sz, vp]
+    L.pwh_lobpcg_gen.restype = i32
     L.pwh_density_workspace_bytes.argtypes = [vp, i64]
     L.pwh_density_workspace_bytes.restype = sz
     L.pwh_density_accumulate.argtypes = [vp, i64, vp, i64, vp, dbl, vp, vp, sz, vp]
@@ -507,6 +514,23 @@ def chol_ortho(psi: torch.Tensor, hpsi: Optional[torch.Tensor] = None):
     return u.T, int(info.item())
 
 
+def chol_ortho_gen(psi: torch.Tensor, hpsi: Optional[torch.Tensor], spsi: torch.Tensor):
+    """pwh_chol_ortho_gen, in place on psi, spsi (and hpsi): returns (U [row, column], info)."""
+    L = load_library()
+    npw = int(psi.shape[1])
+    p, ld = _block_args(psi, npw, "psi")
+    sp, lds = _block_args(spsi, npw, "spsi")
+    nb = int(psi.shape[0])
+    h, ldh = (None, npw) if hpsi is None else _block_args(hpsi, npw, "hpsi")
+    u = torch.empty((nb, nb), dtype=torch.complex128, device=psi.device)
+    info = torch.zeros(1, dtype=torch.int32, device=psi.device)
+    ws = _ws(psi.device, int(L.pwh_rr_workspace_bytes(npw, nb)))
+    with torch.cuda.device(psi.device):
+        _check(L.pwh_chol_ortho_gen(npw, nb, p, ld, h, ldh, sp, lds, u.data_ptr(), nb, info.data_ptr(), ws.data_ptr(),
+                                    ws.numel(), _stream_ptr(psi.device)), "pwh_chol_ortho_gen")
+    return u.T, int(info.item())
+
+
 def rayleigh_ritz(psi: torch.Tensor, hpsi: torch.Tensor, spsi: Optional[torch.Tensor] = None):
     """pwh_rayleigh_ritz, in place on psi, hpsi (and spsi): returns (lambda (nband,), info)."""
     L = load_library()
@@ -564,6 +588,29 @@ def lobpcg(ham: Ham, psi: torch.Tensor, hpsi: torch.Tensor, nblocks: int, nline:
         _check(L.pwh_lobpcg(ham.handle, nb, int(nblocks), int(nline), float(tol), p, ld, h, ldh, lam.data_ptr(), res.data_ptr(),
                             hist.data_ptr() if hist.numel() else None, info.data_ptr(), ws.data_ptr(), ws.numel(),
                             _stream_ptr(ham.device)), "pwh_lobpcg")
+    return {"lam": lam, "resid": res, "history": hist, "info": int(info.item())}
+
+
+def lobpcg_gen(ham: Ham, psi: torch.Tensor, hpsi: torch.Tensor, spsi: torch.Tensor, nblocks: int, nline: int, tol: float = 0.0):
+    """pwh_lobpcg_gen (Algorithm 11 with the PAW overlap S of the handle), in place on psi / hpsi / spsi: returns the same dict
+    as `lobpcg`."""
+    L = load_library()
+    p, ld = _block_args(psi, ham.npw, "psi")
+    h, ldh = _block_args(hpsi, ham.npw, "hpsi")
+    sp, lds = _block_args(spsi, ham.npw, "spsi")
+    nb = int(psi.shape[0])
+    need = int(L.pwh_lobpcg_gen_workspace_bytes(ham.handle, nb, int(nblocks)))
+    if need == 0:
+        raise PwhamError("pwh_lobpcg_gen_workspace_bytes: nband must be a positive multiple of nblocks")
+    lam = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    res = torch.empty(nb, dtype=torch.float64, device=psi.device)
+    hist = torch.full((int(nblocks), max(int(nline), 0), nb // int(nblocks)), float("nan"), dtype=torch.float64, device=psi.device)
+    info = torch.zeros(1, dtype=torch.int32, device=psi.device)
+    ws = _ws(psi.device, need, tag="lobpcg")
+    with torch.cuda.device(ham.device):
+        _check(L.pwh_lobpcg_gen(ham.handle, nb, int(nblocks), int(nline), float(tol), p, ld, h, ldh, sp, lds, lam.data_ptr(),
+                                res.data_ptr(), hist.data_ptr() if hist.numel() else None, info.data_ptr(), ws.data_ptr(),
+                                ws.numel(), _stream_ptr(ham.device)), "pwh_lobpcg_gen")
     return {"lam": lam, "resid": res, "history": hist, "info": int(info.item())}
 
 

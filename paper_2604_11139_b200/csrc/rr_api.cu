@@ -212,13 +212,14 @@ extern "C" size_t pwh_rr_workspace_bytes(int64_t npw, int64_t nband) {
   return rr_layout(npw, nband).total;
 }
 
-extern "C" int pwh_chol_ortho(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh,
-                              pwh_c128* U, int64_t ldu, int32_t* info, void* ws, size_t ws_bytes, void* stream) {
+static int chol_ortho_impl(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh, pwh_c128* spsi,
+                           int64_t lds, pwh_c128* U, int64_t ldu, int32_t* info, void* ws, size_t ws_bytes, void* stream) {
   if (npw < 1 || nband < 0) return api_fail(PWH_EINVAL, "bad sizes");
   if (nband == 0) return PWH_OK;
   int rc;
   if ((rc = check_block(psi, ld, npw, "psi"))) return rc;
   if (hpsi && ldh < npw) return api_fail(PWH_EINVAL, "hpsi: leading dimension smaller than npw");
+  if (spsi && lds < npw) return api_fail(PWH_EINVAL, "spsi: leading dimension smaller than npw");
   if (U && ldu < nband) return api_fail(PWH_EINVAL, "ldu < nband");
   if (!info) return api_fail(PWH_EINVAL, "info is null");
   const RrWs r = rr_layout(npw, nband);
@@ -228,15 +229,29 @@ extern "C" int pwh_chol_ortho(int64_t npw, int64_t nband, pwh_c128* psi, int64_t
   c128* S = (c128*)(wsb + r.ss);
   c128* W = (c128*)(wsb + r.x);
   RR_TRY(rr_kernels_init());
-  // S = Psi^H Psi (Hermitian), S = U^H U, W = U^-1, Psi <- Psi W, H Psi <- (H Psi) W
-  if ((rc = pwh_gram_herm(npw, nband, psi, ld, psi, ld, (pwh_c128*)S, nband, wsb + r.gram, r.total - r.gram, stream))) return rc;
+  // S_Psi = Psi^H (S Psi) (Hermitian; S = I when spsi is null), S_Psi = U^H U, W = U^-1, then Psi, H Psi, S Psi <- . W
+  if ((rc = pwh_gram_herm(npw, nband, psi, ld, spsi ? spsi : psi, spsi ? lds : ld, (pwh_c128*)S, nband, wsb + r.gram,
+                          r.total - r.gram, stream))) return rc;
   launch_potrf_upper((int)nband, S, nband, info, st);
   if (U) RR_TRY(cudaMemcpy2DAsync(U, (size_t)ldu * sizeof(c128), S, (size_t)nband * sizeof(c128), (size_t)nband * sizeof(c128),
                                   (size_t)nband, cudaMemcpyDeviceToDevice, st));
   launch_trinv_upper((int)nband, S, nband, W, nband, st);
   if ((rc = rotate_inplace(npw, nband, (c128*)psi, ld, W, nband, (c128*)(wsb + r.panel), st))) return rc;
   if (hpsi && (rc = rotate_inplace(npw, nband, (c128*)hpsi, ldh, W, nband, (c128*)(wsb + r.panel), st))) return rc;
+  if (spsi && (rc = rotate_inplace(npw, nband, (c128*)spsi, lds, W, nband, (c128*)(wsb + r.panel), st))) return rc;
   return PWH_OK;
+}
+
+extern "C" int pwh_chol_ortho(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh,
+                              pwh_c128* U, int64_t ldu, int32_t* info, void* ws, size_t ws_bytes, void* stream) {
+  return chol_ortho_impl(npw, nband, psi, ld, hpsi, ldh, nullptr, 0, U, ldu, info, ws, ws_bytes, stream);
+}
+
+extern "C" int pwh_chol_ortho_gen(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh,
+                                  pwh_c128* spsi, int64_t lds, pwh_c128* U, int64_t ldu, int32_t* info, void* ws,
+                                  size_t ws_bytes, void* stream) {
+  if (!spsi) return api_fail(PWH_EINVAL, "spsi is null");
+  return chol_ortho_impl(npw, nband, psi, ld, hpsi, ldh, spsi, lds, U, ldu, info, ws, ws_bytes, stream);
 }
 
 extern "C" int pwh_rayleigh_ritz(int64_t npw, int64_t nband, pwh_c128* psi, int64_t ld, pwh_c128* hpsi, int64_t ldh,

@@ -121,3 +121,90 @@ def test_lobpcg_padded_leading_dimensions_and_errors(gpu):
     with pytest.raises(gpu.PwhamError):
         gpu.lobpcg(ham, dev(w.psi), torch.empty_like(dev(w.psi)), 5, 1)      # 12 bands do not split into 5 blocks
     ham.destroy()
+
+
+# ---- Algorithm 11 with the PAW overlap S (pwh_lobpcg_gen) ---------------------------------------------------------------------
+def gen_setup(gpu, w, seed):
+    off, db, qb = synth.paw_blocks(w.nproj, w.dij, seed=seed)
+    ham = gpu.ham_setup(*ham_args(w))
+    assert gpu.ham_set_paw(ham, off, db, qb) == 0
+    return ham, (w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, w.proj, off, db, qb)
+
+
+def compare_gen(out, ref, y, hy, sy, gargs):
+    from oracle import paw
+    lam, lam_ref = out["lam"].cpu().numpy(), ref["lam"]
+    nb = len(lam_ref)
+    scale = np.abs(lam_ref).max()
+    assert np.abs(lam - lam_ref).max() <= 1e-9 * scale
+    assert np.abs(out["resid"].cpu().numpy() - ref["resid"]).max() <= 1e-8 * scale
+    hist = out["history"].cpu().numpy()
+    for i, per_block in enumerate(ref["history"]):
+        for n, norms in enumerate(per_block):
+            assert np.abs(hist[i, n] - norms).max() <= 1e-8 * scale, (i, n)
+    assert np.abs(y.conj() @ sy.T - np.eye(nb)).max() <= 1e-10 * nb          # Psi^H S Psi = I
+    assert np.abs(y.conj() @ hy.T - np.diag(lam)).max() <= 1e-9 * nb * scale  # Psi^H H Psi = Lambda
+    h_ref, s_ref = paw.apply_hs(*gargs, y)
+    assert np.linalg.norm(hy - h_ref) <= 1e-9 * np.linalg.norm(h_ref)          # hpsi, spsi really are H psi, S psi
+    assert np.linalg.norm(sy - s_ref) <= 1e-9 * np.linalg.norm(s_ref)
+    y_ref, sy_ref = ref["psi"], ref["spsi"]
+    gaps = np.diff(lam_ref)
+    assert gaps.min() > 1e-4 * scale, "test problem has (nearly) degenerate levels: pick another seed"
+    for b in range(nb):                                                      # band by band, up to a phase (S inner product)
+        ph = np.vdot(sy_ref[b], y[b])
+        assert abs(abs(ph) - 1.0) <= 1e-8 / gaps.min() * scale
+        assert np.abs(y[b] - ph / abs(ph) * y_ref[b]).max() <= 1e-8 / gaps.min() * scale
+
+
+@pytest.mark.parametrize("name,nblocks,nline", [("box30", 1, 4), ("box30", 3, 3), ("box48", 2, 3), ("tric", 4, 2), ("tric", 1, 0)])
+def test_lobpcg_gen_matches_oracle(gpu, name, nblocks, nline):
+    import torch
+    w = problem(name)
+    ham, gargs = gen_setup(gpu, w, seed=11)
+    psi = dev(w.psi)
+    hpsi, spsi = torch.empty_like(psi), torch.empty_like(psi)
+    out = gpu.lobpcg_gen(ham, psi, hpsi, spsi, nblocks, nline)
+    ref = lo.lobpcg_gen(*gargs, w.psi, nblocks, nline)
+    assert out["info"] > 0
+    compare_gen(out, ref, psi.cpu().numpy(), hpsi.cpu().numpy(), spsi.cpu().numpy(), gargs)
+    ham.destroy()
+
+
+def test_chol_ortho_gen_matches_oracle(gpu):
+    from oracle import paw
+    w = problem("box30")
+    ham, gargs = gen_setup(gpu, w, seed=12)
+    h_ref, s_ref = paw.apply_hs(*gargs, w.psi)
+    y_ref, hy_ref, sy_ref, u_ref = lo.chol_ortho_gen(w.psi, h_ref, s_ref)
+    psi, hpsi, spsi = dev(w.psi), dev(h_ref), dev(s_ref)
+    u, info = gpu.chol_ortho_gen(psi, hpsi, spsi)
+    assert info == 0
+    # the Cholesky factor with positive diagonal is unique: compare everything element by element
+    assert np.abs(u.cpu().numpy() - u_ref).max() <= 1e-11 * np.abs(u_ref).max()
+    for got, ref in ((psi, y_ref), (hpsi, hy_ref), (spsi, sy_ref)):
+        assert np.linalg.norm(got.cpu().numpy() - ref) <= 1e-10 * np.linalg.norm(ref)
+    y = psi.cpu().numpy()
+    assert np.abs(y.conj() @ spsi.cpu().numpy().T - np.eye(y.shape[0])).max() <= 1e-12 * y.shape[0]
+    ham.destroy()
+
+
+def test_lobpcg_gen_converges_to_the_generalised_spectrum(gpu):
+    import scipy.linalg as sl
+    import torch
+    from oracle import paw
+    w = problem("tric")
+    ham, gargs = gen_setup(gpu, w, seed=13)
+    off, db, qb = gargs[6:]
+    hd = oracle.dense_h(w.lattice, w.kpt, w.fft_dims, w.gvec, w.vloc, None, None)
+    p = w.proj
+    hd = hd + p.T @ paw.blockdiag_dense(off, db) @ p.conj()
+    sd = np.eye(w.npw) + p.T @ paw.blockdiag_dense(off, qb) @ p.conj()
+    ev = sl.eigh(hd, sd, eigvals_only=True)[: w.psi.shape[0]]
+    psi = dev(w.psi)
+    hpsi, spsi = torch.empty_like(psi), torch.empty_like(psi)
+    out = gpu.lobpcg_gen(ham, psi, hpsi, spsi, 1, 80, tol=1e-6)
+    assert out["resid"].cpu().numpy().max() <= 2e-6
+    assert np.abs(out["lam"].cpu().numpy() - ev).max() <= 1e-9 * np.abs(ev).max()
+    with pytest.raises(gpu.PwhamError):
+        gpu.lobpcg_gen(ham, psi, hpsi, spsi, 5, 1)
+    ham.destroy()

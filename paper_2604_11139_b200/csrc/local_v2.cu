@@ -82,17 +82,27 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
   //      same index shift as in the x direction, so only q < LQY can hold a row of the disc), input straight from the disc
   {
     const int nitems = R2Y * nxl;
-    for (int i = tid; i < nitems; i += NT) {
+    // the disc comes from L2 / HBM: the loads of a thread's next item are issued before its current item is transformed
+    auto load_item = [&](int i, c128* dstv) {
       uint32_t s, l;
       P.div_nxl.divmod((uint32_t)i, s, l);
-      c128 v[R1Y];
       const int2* yr = yrow + s;
 #pragma unroll
       for (int q = 0; q < LQY; ++q) {
         const int2 row = yr[q * R2Y];
         const uint32_t d = l - (uint32_t)(row.y & 0xffff);
-        v[q] = plane[d < (uint32_t)(row.y >> 16) ? row.x + (int)l : zcol];   // zcol: a padding column, always zero
+        dstv[q] = plane[d < (uint32_t)(row.y >> 16) ? row.x + (int)l : zcol];   // zcol: a padding column, always zero
       }
+    };
+    c128 nxt[LQY];
+    if (tid < nitems) load_item(tid, nxt);
+    for (int i = tid; i < nitems; i += NT) {
+      uint32_t s, l;
+      P.div_nxl.divmod((uint32_t)i, s, l);
+      c128 v[R1Y];
+#pragma unroll
+      for (int q = 0; q < LQY; ++q) v[q] = nxt[q];
+      if (i + NT < nitems) load_item(i + NT, nxt);
       DftPrunedIn<R1Y, +1, LQY>::run(v);
       const c128* tw = twAy + s * (R1Y + 1);
       c128* dst = half + l * YS + s;

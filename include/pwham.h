@@ -18,7 +18,9 @@
  *     thread-local message for the last failure.  Device work is enqueued on `stream` (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream) and is asynchronous: results are valid once the caller has
  *     synchronised that stream.  The *_host entry points synchronise before returning.
- *   - One handle may be used from one stream at a time.  There is no CPU fallback of any kind.
+ *   - One handle may be used from one stream at a time.  There is no CPU fallback of any kind.  Internally a handle may run
+ *     the band groups of the local-potential stage on two private non-blocking streams; they are forked from and joined to
+ *     `stream` by events inside the call, so the caller sees ordinary in-stream semantics.
  *   - Several handles may be alive at once (one per k-point is the normal use); they share nothing.
  *
  * Environment switches.  They exist for the test-suite, select a KERNEL FAMILY (never a CPU path), are sampled once per

@@ -65,7 +65,10 @@ __global__ void __launch_bounds__(C::NT, C::MINB) kv2_plane(const V2Plan P, c128
   c128* twBy = twAy + C::TWA_Y;
   int2* yrow = reinterpret_cast<int2*>(twBy + C::TWB_Y);     // [N2]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int zslot = blockIdx.x, band = blockIdx.y;
+  // CTAs are dispatched in increasing blockIdx.y: walk the bands of the group from the LAST to the first.  The scatter kernel
+  // wrote the column buffer first band first, so what the L2 still holds of a buffer larger than itself is the last bands;
+  // this kernel leaves the first bands in L2, which is where the gather kernel starts.
+  const int zslot = blockIdx.x, band = (int)gridDim.y - 1 - (int)blockIdx.y;
 
   for (int i = tid; i < C::TWA_X; i += NT) twAx[i] = P.twA[0][i];
   for (int i = tid; i < C::TWB_X; i += NT) twBx[i] = P.twB[0][i];

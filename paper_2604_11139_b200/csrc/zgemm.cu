@@ -275,8 +275,10 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm,
       : "memory");
 }
 
-template <bool A_KMAJOR, int EPI, int BK_, int STAGES_>
-__global__ void __launch_bounds__(NT3, 1)
+// JT: 8-column MMA tiles per warp along n -- 2: 16 warps of 32 x 16 (the shape measured throughout); 4: 8 warps of 32 x 32
+// (fewer fragment loads and operand sums per DMMA, 192 accumulator registers)
+template <bool A_KMAJOR, int EPI, int BK_, int STAGES_, int JT = 2>
+__global__ void __launch_bounds__(NT3 * 2 / JT, 1)
 k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int M, int N, int64_t K,
               int tiles_m, int64_t k_per_split, c128* __restrict__ C, int64_t ldc, double alpha, int herm) {
   constexpr int BK = BK_, STAGES = STAGES_, SS = BK / 8;        // SS sub-slabs of 8 k per stage
@@ -284,6 +286,7 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   constexpr int A_BYTES = SS * A_SUB, STAGE_BYTES = SS * (A_SUB + B_SUB);
   extern __shared__ __align__(1024) unsigned char smem[];
   const uint32_t smem_base = ((uint32_t)__cvta_generic_to_shared(smem) + 1023u) & ~1023u;
+  constexpr int NW = 16 * 2 / JT;                                // warps of the CTA
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp % W3_M, wn = warp / W3_M;
   int tm, tn;
@@ -300,7 +303,7 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   const uint32_t bar_full = smem_base + STAGES * STAGE_BYTES, bar_empty = bar_full + STAGES * 8;
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NT3 / 32); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NW); }
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
@@ -326,11 +329,11 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
       if (s < nkt) issue_slab(s, s);
   }
 
-  double t1[4][2][2], t2[4][2][2], t3[4][2][2];
+  double t1[4][JT][2], t2[4][JT][2], t3[4][JT][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 2; ++j)
+    for (int j = 0; j < JT; ++j)
 #pragma unroll
       for (int h = 0; h < 2; ++h) { t1[i][j][h] = 0.0; t2[i][j][h] = 0.0; t3[i][j][h] = 0.0; }
 
@@ -340,7 +343,7 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   // 1024-byte aligned
   const uint32_t a_off0 = A_KMAJOR ? (uint32_t)((wm * 32 + frow) * 128 + (((2 * fk) ^ frow) * 16))
                                    : (uint32_t)((wm * 4) * (BK * 128) + (2 * fk) * 128 + ((frow ^ (2 * fk)) * 16));
-  const uint32_t b_off0 = (uint32_t)(A_BYTES + (wn * 16 + frow) * 128 + (((2 * fk) ^ frow) * 16));
+  const uint32_t b_off0 = (uint32_t)(A_BYTES + (wn * (8 * JT) + frow) * 128 + (((2 * fk) ^ frow) * 16));
   constexpr uint32_t A_ODD = A_KMAJOR ? 16u : (16u | 128u), B_ODD = 16u;
 
   for (int kt = 0; kt < nkt; ++kt) {
@@ -350,16 +353,16 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
 #pragma unroll
     for (int k4 = 0; k4 < BK / 4; ++k4) {
       const int ss = k4 >> 1, par = k4 & 1;
-      double2 b[2];
-      double sb[2];
+      double2 b[JT];
+      double sb[JT];
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < JT; ++j) {
         b[j] = lds128(((st + b_off0) ^ (par ? B_ODD : 0u)) + (uint32_t)(ss * B_SUB + j * 8 * 128));
         sb[j] = b[j].x + b[j].y;
       }
       if (k4 == 0) {
         const int nk = kt + STAGES - 1;
-        if (nk < nkt && warp == (kt & 15)) {
+        if (nk < nkt && warp == (kt & (NW - 1))) {
           if (kt >= 1) mbar_wait(bar_empty + 8 * (nk % STAGES), (uint32_t)((kt - 1) / STAGES) & 1u);
           issue_slab(nk % STAGES, nk);
         }
@@ -371,7 +374,7 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
         const double2 a = lds128(((st + a_off0) ^ (par ? A_ODD : 0u)) + ao);
         const double sa = A_KMAJOR ? a.x - a.y : a.x + a.y;
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
+        for (int j = 0; j < JT; ++j) {
           dmma(t1[i][j][0], t1[i][j][1], a.x, b[j].x);
           dmma(t2[i][j][0], t2[i][j][1], a.y, b[j].y);
           dmma(t3[i][j][0], t3[i][j][1], sa, sb[j]);
@@ -389,10 +392,10 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
     const int m = m0 + wm * 32 + i * 8 + frow;
     if (m >= M) continue;
 #pragma unroll
-    for (int j = 0; j < 2; ++j) {
+    for (int j = 0; j < JT; ++j) {
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        const int n = n0 + wn * 16 + j * 8 + 2 * fk + h;
+        const int n = n0 + wn * (8 * JT) + j * 8 + 2 * fk + h;
         if (n >= N) continue;
         const double re = A_KMAJOR ? t1[i][j][h] + t2[i][j][h] : t1[i][j][h] - t2[i][j][h];
         const double im = A_KMAJOR ? (t3[i][j][h] - t1[i][j][h]) + t2[i][j][h] : (t3[i][j][h] - t1[i][j][h]) - t2[i][j][h];
@@ -463,6 +466,10 @@ constexpr int smem_tma(int bk, int stages) { return stages * (bk / 8) * (BM + BN
 constexpr int smem_cn3() { return CN3_STAGES * (Tile3<CN3_BK>::A_K + Tile3<CN3_BK>::B_) + 2 * CN3_STAGES * 8; }
 constexpr int smem_nn3() { return NN3_STAGES * (Tile3<NN3_BK>::A_M + Tile3<NN3_BK>::B_) + 2 * NN3_STAGES * 8; }
 constexpr int NUM_SMS = 148;
+// warp-tile shapes of the TMA kernels (measured, profiles/r02j): 8 warps of 32 x 32 for CN (-3.3 % at cfg 5: fewer fragment
+// loads and operand sums per DMMA), 16 warps of 32 x 16 for NN (the 32 x 32 shape is 1-5 % slower there: its accumulating epilogue
+// and M-major A fragments want the extra warps)
+constexpr int ZJT_CN = 4, ZJT_NN = 2;
 
 }  // namespace
 
@@ -510,11 +517,11 @@ void zgemm_make_proj_maps(ProjMaps& pm, const c128* P, int64_t npw, int64_t npro
 }
 
 cudaError_t zgemm_init() {
-  cudaError_t e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES>));
+  cudaError_t e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES, ZJT_CN>));
   if (e != cudaSuccess) return e;
-  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES>));
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES, ZJT_NN>));
   if (e != cudaSuccess) return e;
-  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<false, EPI_STORE, NNT_BK, NNT_STAGES>));
+  e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m_tma<false, EPI_STORE, NNT_BK, NNT_STAGES, ZJT_NN>));
   if (e != cudaSuccess) return e;
   e = set_max_dyn_smem(reinterpret_cast<const void*>(&k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES>));
   if (e != cudaSuccess) return e;
@@ -624,7 +631,7 @@ void launch_zgemm_cn(int64_t M, int64_t N, int64_t K, const c128* A, int64_t lda
       else tma = tma && make_map(&tmB, Bk, K, Nk, ldbk, BN);
     }
     if (tma)
-      k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES><<<grid, NT3, smem_tma(CNT_BK, CNT_STAGES), st>>>(
+      k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES, ZJT_CN><<<grid, NT3 * 2 / ZJT_CN, smem_tma(CNT_BK, CNT_STAGES), st>>>(
           tmA, tmB, (int)Mk, (int)Nk, K, tiles_m, kps, part, Mk, 0.0, herm ? 1 : 0);
     else
       k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES><<<grid, NT3, smem_cn3(), st>>>(
@@ -650,10 +657,10 @@ void launch_zgemm_nn(int64_t M, int64_t N, int64_t K, double alpha, const c128* 
   else tma = make_map(&tmA, A, M, K, lda, NNT_BK);
   tma = tma && make_map(&tmB, B, K, N, ldb, BN);
   if (tma && accumulate)
-    k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES><<<grid, NT3, smem_tma(NNT_BK, NNT_STAGES), st>>>(
+    k_zgemm3m_tma<false, EPI_ACC, NNT_BK, NNT_STAGES, ZJT_NN><<<grid, NT3 * 2 / ZJT_NN, smem_tma(NNT_BK, NNT_STAGES), st>>>(
         tmA, tmB, (int)M, (int)N, K, tiles_m, K, C, ldc, alpha, 0);
   else if (tma)
-    k_zgemm3m_tma<false, EPI_STORE, NNT_BK, NNT_STAGES><<<grid, NT3, smem_tma(NNT_BK, NNT_STAGES), st>>>(
+    k_zgemm3m_tma<false, EPI_STORE, NNT_BK, NNT_STAGES, ZJT_NN><<<grid, NT3 * 2 / ZJT_NN, smem_tma(NNT_BK, NNT_STAGES), st>>>(
         tmA, tmB, (int)M, (int)N, K, tiles_m, K, C, ldc, alpha, 0);
   else if (accumulate)
     k_zgemm3m<false, EPI_ACC, NN3_BK, NN3_STAGES><<<grid, NT3, smem_nn3(), st>>>(

@@ -133,6 +133,21 @@ int pwh_gram_herm(int64_t npw, int64_t n, const pwh_c128* X, int64_t ldx, const 
                   int64_t ldg, void* ws, size_t ws_bytes, void* stream);
 
 /*
+ * pwh_gram_static -- pwh_gram for callers that may not allocate and have no workspace to give (code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): G = X^H Y with the split-K partial sums in a file-scope device array of
+ * PWH_GRAM_STATIC_MAX_ENTRIES complex128 (16 MiB; every GPU that loads the library holds it until exit).  Same arguments,
+ * layout and result as pwh_gram, to rounding order (the number of K splits is capped so that the partial sums fit).
+ *   Limit: nx * ny <= PWH_GRAM_STATIC_MAX_ENTRIES, otherwise PWH_EINVAL with a message naming the limit.
+ *   The call performs no cudaMalloc / cudaFree and calls no allocating library routine; it enqueues two kernels on `stream`.
+ *   All calls share the one array, which keeps the previous call's contents (nothing in it needs clearing: every partial entry
+ *   is written before it is read): calls that can overlap on the GPU -- different streams, several host threads -- RACE on it.
+ *   Keep them on one stream or order them with events.
+ */
+#define PWH_GRAM_STATIC_MAX_ENTRIES 1048576
+int pwh_gram_static(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny, const pwh_c128* Y, int64_t ldy,
+                    pwh_c128* G, int64_t ldg, void* stream);
+
+/*
  * Host-buffer entry points (end-to-end path: the paper keeps Psi on the device and moves it host->device once per
  * k-point and SCF step, Algorithm 3).  All pointers below marked HOST are host memory (pinned
  * memory gives asynchronous copies; pageable memory works).  Device staging buffers are allocated on first use,

@@ -30,7 +30,7 @@ EXPORTS = ["pwh_ham_setup", "pwh_ham_destroy", "pwh_workspace_bytes", "pwh_apply
            "pwh_ham_set_paw", "pwh_apply_hs", "pwh_apply_sinv", "pwh_cheb_filter_gen",
            "pwh_lobpcg_workspace_bytes", "pwh_lobpcg",
            "pwh_density_workspace_bytes", "pwh_density_accumulate",
-           "pwh_chol_ortho_gen", "pwh_lobpcg_gen_workspace_bytes", "pwh_lobpcg_gen"]
+           "pwh_chol_ortho_gen", "pwh_lobpcg_gen_workspace_bytes", "pwh_lobpcg_gen", "pwh_gram_static"]
 
 STAGES = ["scatter_zinv", "plane", "zfwd_gather", "zgemm_cn", "splitk_reduce", "zgemm_nn", "colstats", "dense_small",
           "jacobi", "axpy", "reserved10", "reserved11"]
@@ -67,6 +67,8 @@ def load_library() -> ctypes.CDLL:
     L.pwh_gram.argtypes = [i64, i64, vp, i64, i64, vp, i64, vp, i64, vp, sz, vp]
     L.pwh_gram.restype = i32
     L.pwh_gram_herm.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64, vp, sz, vp]
+    L.pwh_gram_static.argtypes = [i64, i64, vp, i64, i64, vp, i64, vp, i64, vp]
+    L.pwh_gram_static.restype = i32
     L.pwh_gram_herm.restype = i32
     L.pwh_ham_kernels.argtypes = [vp, ctypes.c_char_p, sz]
     L.pwh_ham_kernels.restype = i32
@@ -325,6 +327,28 @@ def gram(x: torch.Tensor, y: torch.Tensor, hermitian: bool = False) -> torch.Ten
                             _stream_ptr(x.device))
     _check(rc, "pwh_gram_herm" if hermitian else "pwh_gram")
     return g_cm.T
+
+
+GRAM_STATIC_MAX_ENTRIES = 1048576      # PWH_GRAM_STATIC_MAX_ENTRIES of include/pwham.h
+
+
+def gram_static(x: torch.Tensor, y: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """pwh_gram_static: G = X^H Y with the split-K scratch in the library's static device array (no workspace, no allocation
+    inside the call; nx * ny <= GRAM_STATIC_MAX_ENTRIES).  `out`: optional (ny, nx) complex128 CUDA tensor that receives the
+    column-major result, so that the binding allocates nothing either; returns G of shape (nx, ny)."""
+    L = load_library()
+    npw = int(x.shape[1])
+    x_ptr, ldx = _block_args(x, npw, "x")
+    y_ptr, ldy = _block_args(y, npw, "y")
+    nx, ny = int(x.shape[0]), int(y.shape[0])
+    if out is None:
+        out = torch.empty((ny, nx), dtype=torch.complex128, device=x.device)
+    elif not (out.is_cuda and out.dtype == torch.complex128 and tuple(out.shape) == (ny, nx) and out.is_contiguous()):
+        raise PwhamError("out must be a contiguous CUDA complex128 tensor of shape (ny, nx)")
+    with torch.cuda.device(x.device):
+        rc = L.pwh_gram_static(npw, nx, x_ptr, ldx, ny, y_ptr, ldy, out.data_ptr(), nx, _stream_ptr(x.device))
+    _check(rc, "pwh_gram_static")
+    return out.T
 
 
 def _host_block(a, npw: int, name: str):

@@ -671,3 +671,84 @@ void launch_zgemm_nn(int64_t M, int64_t N, int64_t K, double alpha, const c128* 
 }
 
 }  // namespace pwh
+
+// ---------------------------------------------------------------------------------------------------------------
+// pwh_gram_static -- the Gram product for callers that may not allocate (include/pwham.h): the split-K partial sums that
+// pwh_gram keeps in a caller-provided workspace live in a file-scope device array of fixed size instead.  The array exists
+// once per GPU that loads the library and is shared by every call: calls that overlap on the GPU race on it.  Nothing in it
+// has to start at zero -- the CN kernel writes every partial entry of every split before the reduction reads it.
+// ---------------------------------------------------------------------------------------------------------------
+#include <mutex>
+
+#include "../../include/pwham.h"
+
+static_assert(PWH_GRAM_STATIC_MAX_ENTRIES == 1048576, "keep include/pwham.h and the scratch array in step");
+constexpr size_t GRAM_STATIC_BYTES = (size_t)PWH_GRAM_STATIC_MAX_ENTRIES * sizeof(pwh::c128);     // 16 MiB
+static __device__ __align__(256) unsigned char g_gram_static_scratch[GRAM_STATIC_BYTES];
+
+// device address of the array on the current device: its name is only a host-side stand-in here, so the address is asked
+// for once per device, with that device current
+static cudaError_t gram_static_scratch(void** out) {
+  constexpr int MAXDEV = 64;
+  static std::mutex mu;
+  static void* addr[MAXDEV] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= MAXDEV) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_gram_static_scratch);
+    if (e != cudaSuccess) return e;
+    addr[dev] = p;
+  }
+  *out = addr[dev];
+  return cudaSuccess;
+}
+
+extern "C" int pwh_gram_static(int64_t npw, int64_t nx, const pwh_c128* X, int64_t ldx, int64_t ny, const pwh_c128* Y,
+                               int64_t ldy, pwh_c128* G, int64_t ldg, void* stream) {
+  using namespace pwh;
+  if (npw < 1 || nx < 0 || ny < 0) return api_fail(PWH_EINVAL, "bad sizes");
+  if (nx == 0 || ny == 0) return PWH_OK;
+  if (!X || !Y || !G) return api_fail(PWH_EINVAL, "null argument");
+  if (ldx < npw || ldy < npw || ldg < nx) return api_fail(PWH_EINVAL, "leading dimension too small");
+  if (nx > PWH_GRAM_STATIC_MAX_ENTRIES || ny > PWH_GRAM_STATIC_MAX_ENTRIES || nx * ny > (int64_t)PWH_GRAM_STATIC_MAX_ENTRIES)
+    return api_fail(PWH_EINVAL, "pwh_gram_static: nx * ny = %lld exceeds the static scratch of %lld entries (use pwh_gram)",
+                    (long long)(nx * ny), (long long)PWH_GRAM_STATIC_MAX_ENTRIES);
+  cudaError_t e = zgemm_init();
+  if (e != cudaSuccess) return api_fail(PWH_ECUDA, "zgemm_init: %s", cudaGetErrorString(e));
+  void* scratch = nullptr;
+  e = gram_static_scratch(&scratch);
+  if (e != cudaSuccess) return api_fail(PWH_ECUDA, "cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t M = nx, N = ny, K = npw;
+  // as many K splits as pwh_gram would take, capped so that the partial sums fit the array (at least one always does)
+  int nsplit = zgemm_cn_splits(M, N, K, false);
+  const int64_t cap = (int64_t)PWH_GRAM_STATIC_MAX_ENTRIES / (M * N);
+  if (nsplit > cap) nsplit = (int)cap;
+  const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
+  int64_t kps = (K + nsplit - 1) / nsplit;
+  kps = (kps + CNT_BK - 1) / CNT_BK * CNT_BK;
+  dim3 grid((unsigned)(tiles_m * tiles_n), (unsigned)nsplit);
+  c128* part = reinterpret_cast<c128*>(scratch);
+  const c128 *A = reinterpret_cast<const c128*>(X), *B = reinterpret_cast<const c128*>(Y);
+  CUtensorMap tmA, tmB;
+  count_launch();
+  if (make_map(&tmA, A, K, M, ldx, BM) && make_map(&tmB, B, K, N, ldy, BN))
+    k_zgemm3m_tma<true, EPI_PARTIAL, CNT_BK, CNT_STAGES, ZJT_CN><<<grid, NT3 * 2 / ZJT_CN, smem_tma(CNT_BK, CNT_STAGES), st>>>(
+        tmA, tmB, (int)M, (int)N, K, tiles_m, kps, part, M, 0.0, 0);
+  else
+    k_zgemm3m<true, EPI_PARTIAL, CN3_BK, CN3_STAGES><<<grid, NT3, smem_cn3(), st>>>((int)M, (int)N, K, tiles_m, kps, A, ldx, B, ldy,
+                                                                                   part, M, 0.0, 0);
+  const int64_t total = M * N;
+  int blocks = (int)((total + 255) / 256);
+  if (blocks > NUM_SMS * 8) blocks = NUM_SMS * 8;
+  count_launch();
+  k_splitk_reduce<<<blocks, 256, 0, st>>>((int)M, (int)N, nsplit, part, nullptr, reinterpret_cast<c128*>(G), ldg, 0, 0);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return api_fail(PWH_ECUDA, "pwh_gram_static launch: %s", cudaGetErrorString(e));
+  return PWH_OK;
+}
+

@@ -28,6 +28,10 @@ namespace pwh {
 namespace {
 
 constexpr int ZW = 8;   // warps per CTA; two CTAs per SM
+#ifndef PWH_Z_GATHER_BATCH
+#define PWH_Z_GATHER_BATCH 3
+#endif
+constexpr int ZGB = PWH_Z_GATHER_BATCH;   // entries of the gather epilogue whose loads are issued together
 
 template <int R>
 using RC = std::integral_constant<int, R>;
@@ -100,7 +104,7 @@ __device__ __forceinline__ void scatter_pass1(const int4* __restrict__ tab4, con
 }
 
 // pass 2 of kz_zfwd_gather for one work item: radix R over positions q r2 + sub, outputs q < L, recurrence epilogue
-template <int R, int L>
+template <int R, int L, int GB>
 __device__ __forceinline__ void gather_pass2(const int4* __restrict__ tab4, const c128* __restrict__ src,
                                              const c128* __restrict__ buf, int64_t pstride, int r2, int cw, int lcw, int zs,
                                              int lane, const c128* yb, const c128* pb, c128* ob,
@@ -119,19 +123,52 @@ __device__ __forceinline__ void gather_pass2(const int4* __restrict__ tab4, cons
       for (int q = 0; q < R; ++q) v[q] = b[q * (r2 + 1)];
     }
     Dft<R, -1>::run(v);
+    // `out` may be the buffer of y or y_prev, so the compiler cannot move the loads of one entry above the store of the one
+    // before: entries are handled GB at a time, all loads of a batch first (a thread only ever reads the entries it writes).
+    // GB = 3 in the kernels specialised for one factorisation (what their 128 registers hold), 1 in the generic kernel.
+    if constexpr (GB <= 1) {
 #pragma unroll
-    for (int q = 0; q < L; ++q) {
-      const int g = idx[q];
-      if (g < 0) continue;
-      const c128 yv = yb[g];
-      const double k = kin[g] - cshift;
-      c128 r = cmake(alpha * fma(k, yv.x, v[q].x), alpha * fma(k, yv.y, v[q].y));
-      if (pb) {
-        const c128 pv = pb[g];
-        r.x = fma(-beta, pv.x, r.x);
-        r.y = fma(-beta, pv.y, r.y);
+      for (int q = 0; q < L; ++q) {
+        const int g = idx[q];
+        if (g < 0) continue;
+        const c128 yv = yb[g];
+        const double k = kin[g] - cshift;
+        c128 r = cmake(alpha * fma(k, yv.x, v[q].x), alpha * fma(k, yv.y, v[q].y));
+        if (pb) {
+          const c128 pv = pb[g];
+          r.x = fma(-beta, pv.x, r.x);
+          r.y = fma(-beta, pv.y, r.y);
+        }
+        ob[g] = r;
       }
-      ob[g] = r;
+      continue;
+    }
+#pragma unroll
+    for (int q0 = 0; q0 < L; q0 += GB) {
+      c128 yv[GB], pv[GB];
+      double kk[GB];
+#pragma unroll
+      for (int t = 0; t < GB; ++t) {
+        const int g = q0 + t < L ? idx[q0 + t < L ? q0 + t : 0] : -1;
+        if (g < 0) continue;
+        yv[t] = yb[g];
+        kk[t] = kin[g];
+        if (pb) pv[t] = pb[g];
+      }
+#pragma unroll
+      for (int t = 0; t < GB; ++t) {
+        if (q0 + t >= L) continue;
+        const int q = q0 + t < L ? q0 + t : 0;
+        const int g = idx[q];
+        if (g < 0) continue;
+        const double k = kk[t] - cshift;
+        c128 r = cmake(alpha * fma(k, yv[t].x, v[q].x), alpha * fma(k, yv[t].y, v[q].y));
+        if (pb) {
+          r.x = fma(-beta, pv[t].x, r.x);
+          r.y = fma(-beta, pv[t].y, r.y);
+        }
+        ob[g] = r;
+      }
     }
   }
 }
@@ -248,7 +285,7 @@ __global__ void __launch_bounds__(ZW * 32, 2) kz_zfwd_gather(const ZPlan P, cons
     // are outside the sphere, never used, and their butterflies are dropped); recurrence epilogue
     auto pass2 = [&](auto rc) {
       constexpr int R = decltype(rc)::value;
-      gather_pass2<R, PR ? pruned_len(R) : R>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
+      gather_pass2<R, PR ? pruned_len(R) : R, (R1C > 0 ? ZGB : 1)>(tab4, src, buf, pstride, r2, cw, lcw, zs, lane, yb, pb, ob, kin, alpha, cshift, beta);
     };
     if constexpr (R1C > 0) pass2(RC<R1C>()); else with_radix<true>(r1, pass2);
     __syncwarp();

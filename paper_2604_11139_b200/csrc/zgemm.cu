@@ -345,22 +345,6 @@ k_zgemm3m_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
                                    : (uint32_t)((wm * 4) * (BK * 128) + (2 * fk) * 128 + ((frow ^ (2 * fk)) * 16));
   const uint32_t b_off0 = (uint32_t)(A_BYTES + (wn * (8 * JT) + frow) * 128 + (((2 * fk) ^ frow) * 16));
   constexpr uint32_t A_ODD = A_KMAJOR ? 16u : (16u | 128u), B_ODD = 16u;
-#ifdef PWH_ZGEMM_PREFETCH_C
-  if (EPI == EPI_ACC) {
-    // the tile of C this CTA accumulates onto comes from HBM: start it towards L2 now, the k loop runs meanwhile
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int m = m0 + wm * 32 + i * 8 + frow;
-#pragma unroll
-      for (int j = 0; j < JT; ++j)
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int n = n0 + wn * (8 * JT) + j * 8 + 2 * fk + h;
-          if (m < M && n < N) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(C + (int64_t)n * ldc + m));
-        }
-    }
-  }
-#endif
 
   for (int kt = 0; kt < nkt; ++kt) {
     const int stage = kt % STAGES;

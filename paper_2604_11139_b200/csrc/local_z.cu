@@ -141,33 +141,33 @@ __device__ __forceinline__ void gather_pass2(const int4* __restrict__ tab4, cons
         }
         ob[g] = r;
       }
-      continue;
-    }
+    } else {
 #pragma unroll
-    for (int q0 = 0; q0 < L; q0 += GB) {
-      c128 yv[GB], pv[GB];
-      double kk[GB];
+      for (int q0 = 0; q0 < L; q0 += GB) {
+        c128 yv[GB], pv[GB];
+        double kk[GB];
 #pragma unroll
-      for (int t = 0; t < GB; ++t) {
-        const int g = q0 + t < L ? idx[q0 + t < L ? q0 + t : 0] : -1;
-        if (g < 0) continue;
-        yv[t] = yb[g];
-        kk[t] = kin[g];
-        if (pb) pv[t] = pb[g];
-      }
-#pragma unroll
-      for (int t = 0; t < GB; ++t) {
-        if (q0 + t >= L) continue;
-        const int q = q0 + t < L ? q0 + t : 0;
-        const int g = idx[q];
-        if (g < 0) continue;
-        const double k = kk[t] - cshift;
-        c128 r = cmake(alpha * fma(k, yv[t].x, v[q].x), alpha * fma(k, yv[t].y, v[q].y));
-        if (pb) {
-          r.x = fma(-beta, pv[t].x, r.x);
-          r.y = fma(-beta, pv[t].y, r.y);
+        for (int t = 0; t < GB; ++t) {
+          const int g = q0 + t < L ? idx[q0 + t < L ? q0 + t : 0] : -1;
+          if (g < 0) continue;
+          yv[t] = yb[g];
+          kk[t] = kin[g];
+          if (pb) pv[t] = pb[g];
         }
-        ob[g] = r;
+#pragma unroll
+        for (int t = 0; t < GB; ++t) {
+          if (q0 + t >= L) continue;
+          const int q = q0 + t < L ? q0 + t : 0;
+          const int g = idx[q];
+          if (g < 0) continue;
+          const double k = kk[t] - cshift;
+          c128 r = cmake(alpha * fma(k, yv[t].x, v[q].x), alpha * fma(k, yv[t].y, v[q].y));
+          if (pb) {
+            r.x = fma(-beta, pv[t].x, r.x);
+            r.y = fma(-beta, pv[t].y, r.y);
+          }
+          ob[g] = r;
+        }
       }
     }
   }

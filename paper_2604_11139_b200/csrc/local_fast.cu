@@ -395,11 +395,12 @@ __global__ void __launch_bounds__(PT_MAX, 1) kf_density_plane(const FastPlan P, 
               v[q] = xl >= 0 ? half[xl * ys + y0 + yb] : cmake(0.0, 0.0);
             }
             Dft<R, +1>::run(v);
+            double old[R];
 #pragma unroll
-            for (int q = 0; q < R; ++q) {
-              double* a = az + (int64_t)q * n2 + y0 + yb;
-              *a = fma(f, fma(v[q].x, v[q].x, v[q].y * v[q].y), *a);
-            }
+            for (int q = 0; q < R; ++q) old[q] = az[(int64_t)q * n2 + y0 + yb];
+#pragma unroll
+            for (int q = 0; q < R; ++q)
+              az[(int64_t)q * n2 + y0 + yb] = fma(f, fma(v[q].x, v[q].x, v[q].y * v[q].y), old[q]);
           }
         });
         continue;
@@ -426,8 +427,12 @@ __global__ void __launch_bounds__(PT_MAX, 1) kf_density_plane(const FastPlan P, 
           for (int q = 0; q < R; ++q) v[q] = t[q * YB];
           Dft<R, +1>::run(v);
           double* a = az + (int64_t)(k1 * r2x) * n2 + y0 + yb;
+          // read-modify-write of R entries through one pointer: all loads first, or each load waits for the store before it
+          double old[R];
 #pragma unroll
-          for (int q = 0; q < R; ++q) a[(int64_t)q * n2] = fma(f, fma(v[q].x, v[q].x, v[q].y * v[q].y), a[(int64_t)q * n2]);
+          for (int q = 0; q < R; ++q) old[q] = a[(int64_t)q * n2];
+#pragma unroll
+          for (int q = 0; q < R; ++q) a[(int64_t)q * n2] = fma(f, fma(v[q].x, v[q].x, v[q].y * v[q].y), old[q]);
         }
       });
       __syncthreads();
